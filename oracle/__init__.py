@@ -1,0 +1,28 @@
+"""fp64 CPU oracle for the tomographic reconstruction hot path of arXiv:1806.07938.
+
+THIS PACKAGE IS TEST INFRASTRUCTURE.  Only `tests/`, `__graft_entry__.smoke()` and
+`bench.py`'s `cpu_baseline` / `--impl reference` leg may import it.  It shares no
+code with `paper_1806_07938_b200/` (the CUDA path) and never imports it; the only
+module both sides use is `tomo_inputs/` (seeded inputs, no method arithmetic).
+
+What it computes (each module cites the passage it follows, PAPER.md L<line>):
+
+  vonkarman.py   D_phi(r) of Eq.53 (L619), phase covariance C_phi
+  geometry.py    subaperture / phase-point grids, pupil masks (Fig.2)
+  covariance.py  linear-stencil slope models (Eq.47-48, Eq.54-55), dense C_ss (Eq.14,
+                 L136-158) and C_os (Eq.15-17) built from POSITIONS
+  projectors.py  W, Z, M = I - Z Z^+ (Eq.33-36)
+  solver.py      direct solve of Eq.5/Eq.12 and textbook CG (S2.G L337), Eq.13
+  toeplitz.py    the paper's 2RBT product Eq.18-28 step by step, generators, op counts
+  directsum.py   matrix-free direct-sum MVM for ELT sizes (directsum.c, OpenMP)
+  system.py      assembles a TomoConfig into the operator A, rhs and projections
+
+Pins (tests/test_oracle_*.py, `-m "not gpu"`): closed forms of D_phi, the Kolmogorov
+limit, the PSD integral, printed formulas Eq.50-52 / Eq.56-62 against the generic
+stencil evaluation, symmetry/PSD of C_ss, dense == paper's index maps == 2-D FFT
+product, projector identities, CG -> Cholesky, LGS ground-layer identity, the
+paper's printed closed-form counts (L150, L177, L197, L270, L280, L295).
+
+Parity unpinned: absolute WFE in nm (Table 3), the curves of Fig.9-15 and the FFT
+slope model (Eq.41-46) are not reproduced; nothing in this package depends on them.
+"""
