@@ -1,0 +1,156 @@
+/* tomo.h -- C ABI of libtomo_b200: FFT/Toeplitz MMSE tomographic wave-front reconstruction on one B200.
+ *
+ * The method is Ono et al., arXiv:1806.07938 (citations below are PAPER.md L<line>, section / equation):
+ * solve  M_s (W_s Sigma_ss W_s^T + Sigma_eta) M_s^T zeta = M_s s   (Eq.12, Eq.34) by a fixed
+ * number of conjugate-gradient iterations (S2.G L337), every covariance product applied through its 2RBT
+ * (block-Toeplitz-Toeplitz-block) structure by zero-padded 2-D FFTs (S2.E L201-270, Eq.18-30), then project
+ * phi_hat = M_phi W_phi Sigma_{phi s} W_s^T M_s^T zeta   (Eq.13, Eq.31 L276 / Eq.32, Eq.35).
+ *
+ * Conventions
+ *   - every call returns int: TOMO_OK (0) or a negative error code; tomo_last_error() gives a thread-local
+ *     message.  No C++ exception crosses this boundary.  There is NO CPU fallback: every entry point that
+ *     computes needs a CUDA device and fails with TOMO_ECUDA without one.
+ *   - "host" / "device" in an argument comment says where the pointer must live.  Host arrays are copied
+ *     before the call returns.  Device arrays and the stream belong to the caller and must stay valid until
+ *     the stream has passed the call; all compute calls are asynchronous on `cuda_stream` (a cudaStream_t
+ *     passed as void*, NULL = the legacy default stream) and never synchronise with the host.
+ *   - slopes layout (Eq.29):
+ *         [frame][wfs][component: x then y][valid subaperture in row-major order of the n x n grid]   fp32
+ *     slope unit = phase difference across a subaperture edge pair divided by d (rad/m; reading G6).
+ *   - wavefront layout (Eq.35):
+ *         [frame][target][valid phase point in row-major order of the (n+1) x (n+1) corner grid]      fp32
+ *     radians of phase at the wavelength r0 is given at.
+ */
+#ifndef TOMO_B200_H
+#define TOMO_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TOMO_OK            0
+#define TOMO_EINVAL       -1   /* bad sizes, fractions not summing to 1 (1e-9), h_k >= h_gs, n_iter < 0, NULL ...   */
+#define TOMO_EUNSUPPORTED -2   /* high-order set mixes NGS/LGS or LGS altitudes (not 2RBT, L158); FFT edge not 2^a3^b5^c */
+#define TOMO_ENOTREADY    -3   /* compute call before tomo_plan_upload_kernels                                        */
+#define TOMO_ENOMEM       -4
+#define TOMO_ECUDA        -5   /* no device, launch or allocation failure                                           */
+
+#define TOMO_HUDGIN 0          /* Eq.47-52 (L584-615), default slope model                                            */
+#define TOMO_FRIED  1          /* Eq.54-62 (L630-691)                                                                 */
+
+#define TOMO_F32       0       /* fp32 storage and arithmetic (headline path)                                         */
+#define TOMO_F32S_F64A 1       /* fp32-stored spectra, fp64 FFT / vectors                                             */
+#define TOMO_F64       2       /* everything fp64 (parity gate P-e); the slope / wavefront ABI stays fp32             */
+
+#define TOMO_SOLVER_MULTIKERNEL 0   /* one kernel per phase, whole solve replayed from a CUDA graph                  */
+#define TOMO_SOLVER_PERSISTENT  1   /* one cooperative persistent kernel per solve, device-side grid barriers        */
+
+typedef struct tomo_plan tomo_plan;          /* opaque; owns every device allocation it makes                        */
+
+typedef struct {
+    double ax, ay;        /* direction alpha_j [arcsec] (L41)                                                        */
+    double h_gs;          /* guide-star altitude [m]; INFINITY = natural guide star (L158)                           */
+    int    n_remove;      /* modes removed from this WFS: 0, 2 (tip/tilt) or 3 (tip/tilt/focus) (L321-329, Eq.36)    */
+} tomo_wfs;
+
+typedef struct {
+    double D;                          /* pupil diameter [m]                                                         */
+    int    n;                          /* subapertures across; d = D/n (Fig.2)                                  */
+    double obstruction;                /* central obstruction ratio (0 = none)                                       */
+    const unsigned char *subap_mask;   /* host, n*n row-major, non-zero = valid; NULL = centre-inside-pupil rule     */
+    int    n_wfs;                      /* high-order WFSs: all NGS, or all LGS at ONE altitude (L158)                */
+    const tomo_wfs *wfs;               /* host [n_wfs]                                                               */
+    int    n_lo;                       /* low-order NGS sensors: validated only, not part of the CG system (L412)    */
+    const tomo_wfs *lo_wfs;            /* host [n_lo] or NULL                                                        */
+    int    n_targets;                  /* science directions beta_t (L41, L132)                                      */
+    const double *target_xy;           /* host [n_targets][2] arcsec, targets at infinity                            */
+} tomo_geometry;
+
+typedef struct {
+    int n_layers;                      /* K                                                                          */
+    const double *h;                   /* host [K] layer altitudes [m]                                               */
+    const double *frac;                /* host [K] Cn2 fractions, sum to 1 (L562)                                    */
+} tomo_cn2;
+
+typedef struct {
+    const double *sigma2_wfs;          /* host [n_wfs] slope-noise variance (Sigma_eta diagonal, L110, L260) or NULL */
+    double noise_frac;                 /* used when sigma2_wfs == NULL: sigma^2 = noise_frac * model slope variance  */
+                                       /* of WFS 0, 1/2 [theta_xx(0) + theta_yy(0)]  (reading G15)                   */
+    const double *sigma2_subap;        /* optional host [n_wfs][2][n_vs] full diagonal; overrides both; NULL if unused */
+} tomo_noise;
+
+typedef struct {
+    int slope_model;                   /* TOMO_HUDGIN | TOMO_FRIED                                                   */
+    int pad;                           /* FFT edge P for Sigma_ss, 0 = next even 2^a 3^b 5^c >= 2n-1   (L207, G11)    */
+    int pad_os;                        /* FFT edge P_os for Sigma_phi-s, 0 = next even 5-smooth >= n'+n-1            */
+    int max_batch;                     /* largest n_frames a solve may be given (>= 1)                               */
+    int precision;                     /* TOMO_F32 | TOMO_F32S_F64A | TOMO_F64                                       */
+    int solver;                        /* TOMO_SOLVER_MULTIKERNEL | TOMO_SOLVER_PERSISTENT                           */
+    int build_cos;                     /* 0 = no target projection (tomo_solve then returns zeta-less zeros: EINVAL) */
+} tomo_options;
+
+/* Validate the problem statement (S2 L41-58; S2.F L297-333), build masks W_s, W_phi (Eq.33-35), modal matrices
+ * Z_s, Z_phi and (Z^T Z)^-1 (Eq.36), cone factors gamma_k and the common n' (L158, L179, L295), choose P, P_os and
+ * allocate every device buffer.  `opt` may be NULL (defaults: Hudgin, automatic pads, batch 1, fp32,
+ * multi-kernel solver, C_os built).  On success *out owns the plan. */
+int tomo_plan_create(const tomo_geometry *geom, const tomo_cn2 *cn2, double r0, double L0,
+                     const tomo_noise *noise, const tomo_options *opt, tomo_plan **out);
+
+/* One-time covariance-kernel builder (L150, L158, L179-197, L265, L295; Eq.50-53).
+ *   css_gen: host fp64 [C][C][2n-1][2n-1] generators theta[(i,a),(j,b)](l), index (ly+n-1, lx+n-1), lag = input - output,
+ *            C = 2 n_wfs, channel = 2*wfs + component; NULL = build from the von Karman structure function.
+ *   cos_gen: host fp64 [T][K'][C][n'+n-1][n'+n-1] generators xi'[t,k,(j,b)](l), l = q - p' in [-(n'-1), n-1]^2,
+ *            K' = n_layers (LGS) or 1 (NGS, layers summed); NULL = build.
+ * Computes the circular embeddings, their 2-D real DFTs in fp64, folds 1/P^2, keeps the Hermitian half and only
+ * blocks (c_out <= c_in), converts to the plan's storage precision and uploads once. */
+int tomo_plan_upload_kernels(tomo_plan *plan, const double *css_gen, const double *cos_gen);
+
+/* Full path A1-A8 for one frame: n_iter CG iterations from a cold start, then the projection to every target.
+ * slopes: device fp32 [C][n_vs]; wavefront_out: device fp32 [n_targets][n_vphi]. */
+int tomo_solve(tomo_plan *plan, const float *slopes, float *wavefront_out, int n_iter, void *cuda_stream);
+
+/* Same for n_frames <= max_batch independent frames; x0 (device fp32 [n_frames][C][n_vs]) is an optional warm
+ * start (L428, L506), NULL = cold start (L490). */
+int tomo_solve_batch(tomo_plan *plan, const float *slopes, float *wavefront_out, int n_frames, int n_iter,
+                     const float *x0, void *cuda_stream);
+
+/* out = M_s (W_s Sigma_ss W_s^T + Sigma_eta) M_s^T v  (Eq.30, Eq.34): one product, for the MVM gate.
+ * v, out: device fp32 [C][n_vs]. */
+int tomo_apply_css(tomo_plan *plan, const float *v, float *out, void *cuda_stream);
+
+/* wavefront_out = M_phi W_phi Sigma_{phi s} W_s^T M_s^T zeta  (Eq.31/32, Eq.35) for every target (A7-A8 only).
+ * zeta: device fp32 [C][n_vs]; wavefront_out: device fp32 [n_targets][n_vphi]. */
+int tomo_apply_cos(tomo_plan *plan, const float *zeta, float *wavefront_out, void *cuda_stream);
+
+/* One CG iteration (S2.G L337) on caller-held state, for the teacher-forced gate:
+ * x, r, p: device fp32 [C][n_vs], updated in place; rho_alpha_beta: device fp64 [3]: in [0] = rho_k = r_k.r_k,
+ * out [0] = rho_{k+1}, [1] = alpha_k, [2] = beta_k. */
+int tomo_cg_step(tomo_plan *plan, float *x, float *r, float *p, double *rho_alpha_beta, void *cuda_stream);
+
+/* The CG solution zeta of the last solve: device->device copy into zeta_out (device fp32 [n_frames][C][n_vs]). */
+int tomo_get_zeta(tomo_plan *plan, float *zeta_out, int n_frames, void *cuda_stream);
+
+/* Sizes fixed at plan creation; any pointer may be NULL. */
+int tomo_get_sizes(const tomo_plan *plan, int *n_vs, int *n_vphi, int *slopes_len, int *wavefront_len,
+                   int *pad, int *pad_os, int *n_prime);
+
+/* Row-major grid indices of the valid subapertures ([n_vs], host) and valid phase points ([n_vphi], host). */
+int tomo_get_valid_index(const tomo_plan *plan, int *subap_idx, int *phase_idx);
+
+/* sigma^2 per WFS actually used (host fp64 [n_wfs]) and the model slope variance of WFS 0 (host fp64 [1]). */
+int tomo_get_noise(const tomo_plan *plan, double *sigma2_wfs, double *slope_var);
+
+/* Residual history sqrt(rho_k), k = 0..n_iter of the last solve: host fp64 [n_frames][n_iter+1].  The caller
+ * must have synchronised the stream of that solve; this call copies device->host synchronously. */
+int tomo_get_residuals(const tomo_plan *plan, double *host_out, int n_frames, int n_iter);
+
+/* Bytes of device memory owned by the plan, and the number of kernel launches the last solve enqueued. */
+int tomo_get_stats(const tomo_plan *plan, long long *device_bytes, int *launches_last_solve);
+
+void tomo_plan_destroy(tomo_plan *plan);
+const char *tomo_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TOMO_B200_H */

@@ -1,0 +1,221 @@
+// host_kernels.cpp -- 2RBT generators of Sigma_ss and Sigma_phi-s and their spectra (row A0), fp64 on the host.
+// Citations: PAPER.md L<line>.  Written from the paper; shares nothing with oracle/.
+#include <algorithm>
+#include <cmath>
+#include <limits>
+
+#include "host_model.hpp"
+
+namespace tomo {
+namespace {
+struct Tap { int u, v; double w; };
+
+// Linear slope stencils on the phase, offsets in units of HALF the local subaperture width (App. A):
+//   Hudgin-like Eq.47-48 (L584-594): s_x = c [phi(r + w/2 x^) - phi(r - w/2 x^)]
+//   Fried       Eq.54-55 (L630-640): s_x = c/2 [phi(++) - phi(-+) - phi(--) + phi(+-)]
+std::vector<Tap> stencil(int model, int comp) {
+    if (model == TOMO_FRIED) {
+        if (comp == 0) return {{+1, +1, +0.5}, {-1, +1, -0.5}, {-1, -1, -0.5}, {+1, -1, +0.5}};
+        return {{+1, +1, +0.5}, {-1, +1, +0.5}, {-1, -1, -0.5}, {+1, -1, -0.5}};
+    }
+    if (comp == 0) return {{+1, 0, +1.0}, {-1, 0, -1.0}};
+    return {{0, +1, +1.0}, {0, -1, -1.0}};
+}
+
+std::vector<Tap> pair_stencil(int model, int a, int b) {
+    std::vector<Tap> out;
+    for (const Tap &sa : stencil(model, a))
+        for (const Tap &sb : stencil(model, b)) {
+            const int u = sb.u - sa.u, v = sb.v - sa.v;
+            bool found = false;
+            for (Tap &t : out)
+                if (t.u == u && t.v == v) { t.w += sa.w * sb.w; found = true; }
+            if (!found) out.push_back({u, v, sa.w * sb.w});
+        }
+    out.erase(std::remove_if(out.begin(), out.end(), [](const Tap &t) { return t.w == 0.0; }), out.end());
+    return out;
+}
+
+// D_phi on the half-step lattice {(hx, hy) * half + shift}: each value is needed by several lags and several
+// component pairs (the +-d/2 arms of neighbouring lags coincide), so it is evaluated once.
+struct Lattice {
+    int lo, size;
+    double half, sx, sy, r0, L0;
+    std::vector<double> tab;
+    Lattice(int lo_, int hi_, double half_, double sx_, double sy_, double r0_, double L0_)
+        : lo(lo_), size(hi_ - lo_ + 1), half(half_), sx(sx_), sy(sy_), r0(r0_), L0(L0_),
+          tab((size_t)size * size, std::numeric_limits<double>::quiet_NaN()) {}
+    double get(int hx, int hy) {
+        double &v = tab[(size_t)(hy - lo) * size + (hx - lo)];
+        if (std::isnan(v)) v = structure_function(std::hypot(hx * half + sx, hy * half + sy), r0, L0);
+        return v;
+    }
+};
+}  // namespace
+
+// 1/2 [theta_x0x0(0) + theta_y0y0(0)]: the model slope variance the noise level is quoted against (reading G15)
+double model_slope_variance(const HostModel &m) {
+    double v = 0.0;
+    const double c = 1.0 / m.d;
+    for (int k = 0; k < m.K; ++k) {
+        const double w = m.gamma[k] * m.d;
+        Lattice lat(-2, 2, 0.5 * w, 0.0, 0.0, m.r0, m.L0);
+        for (int a = 0; a < 2; ++a) {
+            double s = 0.0;
+            for (const Tap &t : pair_stencil(m.slope_model, a, a)) s += t.w * lat.get(t.u, t.v);
+            v += m.frac[k] * (-0.5 * c * c) * s;
+        }
+    }
+    return 0.5 * v;
+}
+
+// ------------------------------------------------------------------------------------------------ Sigma_ss
+// theta[(i,a),(j,b)](l) = sum_k f_k cov_ab(gamma_k d l + h_k (alpha_j - alpha_i); d_k)        (L150, L158, L265)
+// cov_ab(Delta; w)      = -1/2 c^2 sum_{m,m'} w_m w'_m' D_phi(|Delta + o'_m' - o_m|), c = 1/d  (Eq.49;
+//                         Eq.50-52 are the Hudgin special cases, Eq.51's last sign corrected -- reading G4)
+void build_css_generators(const HostModel &m, std::vector<double> &gen) {
+    const int n = m.n, N = m.n_wfs, C = m.C, L = 2 * n - 1, K = m.K;
+    const size_t LL = (size_t)L * L;
+    gen.assign((size_t)C * C * LL, 0.0);
+    const double c = 1.0 / m.d;
+    std::vector<Tap> st[2][2];
+    for (int a = 0; a < 2; ++a)
+        for (int b = 0; b < 2; ++b) st[a][b] = pair_stencil(m.slope_model, a, b);
+    // distinct WFS pairs: (0,0) stands for every i == j (zero shift), plus all i < j
+    std::vector<std::pair<int, int>> pairs;
+    pairs.push_back({0, 0});
+    for (int i = 0; i < N; ++i)
+        for (int j = i + 1; j < N; ++j) pairs.push_back({i, j});
+    std::vector<double> tmp((size_t)K * 4 * LL);
+    for (const auto &pr : pairs) {
+        const int i = pr.first, j = pr.second;
+#pragma omp parallel for schedule(dynamic)
+        for (int k = 0; k < K; ++k) {
+            const double w = m.gamma[k] * m.d;
+            const double shx = m.h[k] * (m.ax[j] - m.ax[i]), shy = m.h[k] * (m.ay[j] - m.ay[i]);
+            Lattice lat(-2 * n, 2 * n, 0.5 * w, shx, shy, m.r0, m.L0);
+            const double scale = m.frac[k] * (-0.5 * c * c);
+            for (int a = 0; a < 2; ++a)
+                for (int b = 0; b < 2; ++b) {
+                    double *o = &tmp[((size_t)k * 4 + a * 2 + b) * LL];
+                    for (int ly = -(n - 1); ly < n; ++ly)
+                        for (int lx = -(n - 1); lx < n; ++lx) {
+                            double s = 0.0;
+                            for (const Tap &t : st[a][b]) s += t.w * lat.get(2 * lx + t.u, 2 * ly + t.v);
+                            o[(size_t)(ly + n - 1) * L + (lx + n - 1)] = scale * s;
+                        }
+                }
+        }
+        // layer sum in a fixed order (deterministic), then place the block(s)
+        std::vector<double> acc(4 * LL, 0.0);
+#pragma omp parallel for schedule(static)
+        for (long e = 0; e < (long)(4 * LL); ++e) {
+            double s = 0.0;
+            for (int k = 0; k < K; ++k) s += tmp[(size_t)k * 4 * LL + e];
+            acc[e] = s;
+        }
+        auto place = [&](int wi, int wj) {
+            for (int a = 0; a < 2; ++a)
+                for (int b = 0; b < 2; ++b) {
+                    const int co = 2 * wi + a, ci = 2 * wj + b;
+                    double *dst = &gen[((size_t)co * C + ci) * LL];
+                    double *dstT = &gen[((size_t)ci * C + co) * LL];
+                    const double *src = &acc[(size_t)(a * 2 + b) * LL];
+                    for (size_t e = 0; e < LL; ++e) dst[e] = src[e];
+                    if (wi != wj)   // theta_{(j,b),(i,a)}(l) = theta_{(i,a),(j,b)}(-l)
+                        for (size_t e = 0; e < LL; ++e) dstT[LL - 1 - e] = src[e];
+                }
+        };
+        if (i == j) for (int w = 0; w < N; ++w) place(w, w);
+        else place(i, j);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ Sigma_phi-s
+// xi'[k,(j,b)](l) = f_k cov_phi,b(d_k l + d_k[(n'-1)/2 - (n-1)/2] + h_k (alpha_j - beta); d_k),  l = q - p'
+// cov_phi,b(Delta; w) = -1/2 c sum_m' w'_m' D_phi(|Delta + o'_m'|)            (Eq.52; L179-197; reading G18)
+// NGS systems: gamma_k = 1, n' = n+1, and the layers are summed into one table (Eq.15, Eq.31).
+void build_cos_generators(const HostModel &m, int target, std::vector<double> &gen) {
+    const int n = m.n, np = m.n_p, N = m.n_wfs, C = m.C, Los = np + n - 1, K = m.K;
+    const size_t LL = (size_t)Los * Los;
+    gen.assign((size_t)m.Kp * C * LL, 0.0);
+    const double c = 1.0 / m.d;
+    std::vector<Tap> st[2] = {stencil(m.slope_model, 0), stencil(m.slope_model, 1)};
+    std::vector<double> tmp;
+    if (!m.lgs) tmp.assign((size_t)K * C * LL, 0.0);
+#pragma omp parallel for collapse(2) schedule(dynamic)
+    for (int k = 0; k < K; ++k)
+        for (int j = 0; j < N; ++j) {
+            const double w = m.gamma[k] * m.d;
+            const double off = w * ((np - 1) / 2.0 - (n - 1) / 2.0);
+            const double shx = off + m.h[k] * (m.ax[j] - m.bx[target]);
+            const double shy = off + m.h[k] * (m.ay[j] - m.by[target]);
+            Lattice lat(-2 * np, 2 * n, 0.5 * w, shx, shy, m.r0, m.L0);
+            const double scale = m.frac[k] * (-0.5 * c);
+            for (int b = 0; b < 2; ++b) {
+                double *o = m.lgs ? &gen[((size_t)k * C + 2 * j + b) * LL] : &tmp[((size_t)k * C + 2 * j + b) * LL];
+                for (int ly = -(np - 1); ly < n; ++ly)
+                    for (int lx = -(np - 1); lx < n; ++lx) {
+                        double s = 0.0;
+                        for (const Tap &t : st[b]) s += t.w * lat.get(2 * lx + t.u, 2 * ly + t.v);
+                        o[(size_t)(ly + np - 1) * Los + (lx + np - 1)] = scale * s;
+                    }
+            }
+        }
+    if (!m.lgs) {
+#pragma omp parallel for schedule(static)
+        for (long e = 0; e < (long)((size_t)C * LL); ++e) {
+            double s = 0.0;
+            for (int k = 0; k < K; ++k) s += tmp[(size_t)k * C * LL + e];
+            gen[e] = s;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ host FFT
+// Stockham autosort, radices 2/3/4/5 by direct small DFTs; exact enough (fp64) and only used at plan build.
+void host_fft(std::complex<double> *x, int n, int stride, bool inverse) {
+    typedef std::complex<double> cd;
+    std::vector<cd> a(n), b(n);
+    for (int i = 0; i < n; ++i) a[i] = x[(size_t)i * stride];
+    std::vector<cd> tw(n);
+    const double sgn = inverse ? +1.0 : -1.0;
+    for (int t = 0; t < n; ++t) tw[t] = cd(std::cos(2.0 * M_PI * t / n), sgn * std::sin(2.0 * M_PI * t / n));
+    int ncur = n, s = 1;
+    cd *src = a.data(), *dst = b.data();
+    while (ncur > 1) {
+        int r = (ncur % 4 == 0) ? 4 : (ncur % 2 == 0) ? 2 : (ncur % 3 == 0) ? 3 : 5;
+        const int mm = ncur / r;
+        for (int p = 0; p < mm; ++p)
+            for (int q = 0; q < s; ++q) {
+                cd in[5];
+                for (int j = 0; j < r; ++j) in[j] = src[q + s * (p + mm * j)];
+                for (int k = 0; k < r; ++k) {
+                    cd acc(0, 0);
+                    for (int j = 0; j < r; ++j) acc += in[j] * tw[(size_t)((j * k) % r) * (n / r)];
+                    dst[q + s * (r * p + k)] = acc * tw[(size_t)p * k * s];
+                }
+            }
+        ncur = mm; s *= r;
+        std::swap(src, dst);
+    }
+    for (int i = 0; i < n; ++i) x[(size_t)i * stride] = src[i];
+}
+
+// K[(-l) mod P] = g(l); out = rfft2(K)/P^2 stored [kx][ky]   (L207, L265; readings G10, G24)
+void generator_spectrum(const double *g, int n_out, int n_in, int P, std::complex<double> *out) {
+    typedef std::complex<double> cd;
+    const int Lg = n_out + n_in - 1, Ph = P / 2 + 1;
+    std::vector<cd> img((size_t)P * P, cd(0, 0));
+    for (int ly = -(n_out - 1); ly < n_in; ++ly)
+        for (int lx = -(n_out - 1); lx < n_in; ++lx)
+            img[(size_t)(((-ly) % P + P) % P) * P + (((-lx) % P + P) % P)] = g[(size_t)(ly + n_out - 1) * Lg + (lx + n_out - 1)];
+    for (int y = 0; y < P; ++y) host_fft(&img[(size_t)y * P], P, 1, false);     // along x
+    const double sc = 1.0 / ((double)P * P);
+    for (int kx = 0; kx < Ph; ++kx) {
+        host_fft(&img[kx], P, P, false);                                          // along y
+        for (int ky = 0; ky < P; ++ky) out[(size_t)kx * P + ky] = img[(size_t)ky * P + kx] * sc;
+    }
+}
+
+}  // namespace tomo
