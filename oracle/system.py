@@ -117,6 +117,33 @@ class OracleSystem:
         q = directsum.css_mvm(self.generators(), self.ix, self.iy, u) + self.sigma2 * u
         return self.project_slopes(q)
 
+    def css_rows_explicit(self, rows):
+        """Selected rows of W_s Sigma_ss W_s^T built from POSITIONS exactly as covariance.dense_css does (Eq.14,
+        L158): the row-sampled check that pins the generator / direct-sum route at sizes where the dense matrix does
+        not fit.  rows: flat indices (i, a, q) -> (i*2 + a)*nv + q.  Returns (len(rows), Ns)."""
+        c = self.cfg
+        out = np.zeros((len(rows), self.N, 2, self.nv))
+        for t, row in enumerate(rows):
+            ch, q = divmod(int(row), self.nv)
+            i, a = divmod(ch, 2)
+            for hk, fk in zip(c.h, c.frac):
+                g = geo.cone_factor(hk, self.h_gs)
+                pos_i = g * self.centres[q] + hk * np.asarray(self.dirs[i]) * geo.ARCSEC
+                for j in range(self.N):
+                    pos_j = g * self.centres + hk * np.asarray(self.dirs[j]) * geo.ARCSEC
+                    delta = pos_j - pos_i[None, :]
+                    for b in range(2):
+                        out[t, j, b] += fk * cov.cov_slope_slope(delta, a, b, g * self.d, 1.0 / self.d, c.r0, c.L0,
+                                                                 self.model)
+        return out.reshape(len(rows), self.Ns)
+
+    def css_unprojected(self, u):
+        """W_s Sigma_ss W_s^T u without noise and projectors (dense or direct-sum)."""
+        if self.dense:
+            return self.Css @ u
+        from . import directsum
+        return directsum.css_mvm(self.generators(), self.ix, self.iy, np.asarray(u, dtype=np.float64))
+
     def rhs(self, slopes):
         return self.project_slopes(np.asarray(slopes, dtype=np.float64))
 

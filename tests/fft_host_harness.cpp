@@ -1,0 +1,53 @@
+// CPU harness for csrc/fft_device.cuh: the same template code the kernels use, compiled by g++ with one lane,
+// checked against a direct O(P^2) DFT in fp64.  Prints "P <fwd32> <inv32> <fwd64> <inv64>" per size.
+#include <cmath>
+#include <complex>
+#include <cstdio>
+#include <cstdlib>
+#include <vector>
+
+#include "fft_device.cuh"
+using namespace tomo;
+
+static void plan(int P, FftDesc &d) {
+    d.P = P; d.nrad = 0;
+    int r = P;
+    while (r % 5 == 0) { d.rad[d.nrad++] = 5; r /= 5; }
+    while (r % 3 == 0) { d.rad[d.nrad++] = 3; r /= 3; }
+    while (r % 8 == 0) { d.rad[d.nrad++] = 8; r /= 8; }
+    while (r % 4 == 0) { d.rad[d.nrad++] = 4; r /= 4; }
+    while (r % 2 == 0) { d.rad[d.nrad++] = 2; r /= 2; }
+}
+
+template <typename T> static double run(int P, bool inv) {
+    typedef typename cx_of<T>::type C;
+    FftDesc d;
+    plan(P, d);
+    std::vector<C> a(P), b(P), tw(P);
+    std::vector<std::complex<double>> in(P);
+    for (int i = 0; i < P; ++i) {
+        in[i] = {std::sin(i * 1.3) + 0.01 * i, std::cos(i * 0.7) - 0.3};
+        a[i].x = (T)in[i].real(); a[i].y = (T)in[i].imag();
+        tw[i].x = (T)std::cos(2 * M_PI * i / P); tw[i].y = (T)-std::sin(2 * M_PI * i / P);
+    }
+    C *r = inv ? warp_fft<T, true, 1>(a.data(), b.data(), d, tw.data(), 0) : warp_fft<T, false, 1>(a.data(), b.data(), d, tw.data(), 0);
+    double err = 0, nrm = 0;
+    for (int k = 0; k < P; ++k) {
+        std::complex<double> s = 0;
+        for (int j = 0; j < P; ++j) {
+            const double ph = (inv ? 1 : -1) * 2 * M_PI * (double)(((long)j * k) % P) / P;
+            s += in[j] * std::complex<double>(std::cos(ph), std::sin(ph));
+        }
+        err += std::norm(s - std::complex<double>(r[k].x, r[k].y));
+        nrm += std::norm(s);
+    }
+    return std::sqrt(err / nrm);
+}
+
+int main(int argc, char **argv) {
+    for (int i = 1; i < argc; ++i) {
+        const int P = std::atoi(argv[i]);
+        std::printf("%d %.3e %.3e %.3e %.3e\n", P, run<float>(P, false), run<float>(P, true), run<double>(P, false), run<double>(P, true));
+    }
+    return 0;
+}

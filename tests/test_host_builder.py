@@ -1,0 +1,92 @@
+"""Row A0 on the CPU box: the library's host-side covariance-kernel builder (C++, include/tomo_host.h) against the
+oracle's independent evaluation of the same paper formulas (Eq.50-53)."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+from oracle import toeplitz as tz
+from oracle import vonkarman as vk
+from paper_1806_07938_b200 import tomo
+from tomo_inputs.configs import get_config, small_lgs_config, sweep_config
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _anchors():
+    out = {}
+    for line in open(os.path.join(ROOT, "tests", "golden", "dphi_anchors.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        name, val, r0, L0 = [t.strip() for t in line.split("|")]
+        out[name] = (float(val), float(r0), float(L0))
+    return out
+
+
+def test_structure_function_matches_oracle_anchors_and_limits():
+    a = _anchors()
+    for name, (val, r0, L0) in a.items():
+        if name.startswith("dphi_r"):
+            got = tomo.host_structure_function(np.array([float(name[6:])]), r0, L0)[0]
+            assert abs(got / val - 1) < 1e-10, name
+    r = np.linspace(0.01, 120.0, 500)
+    np.testing.assert_allclose(tomo.host_structure_function(r, 0.15, 25.0), vk.structure_function(r, 0.15, 25.0), rtol=1e-10)
+    assert tomo.host_structure_function(np.array([0.0]), 0.15, 25.0)[0] == 0.0
+    # saturation D(inf) = 0.17262866 (L0/r0)^{5/3} and the Kolmogorov limit 6.8839 (r/r0)^{5/3} for r << L0 (the C++ side
+    # switches to the small-argument series there, reading G23)
+    assert abs(tomo.host_structure_function(np.array([1e4]), 0.15, 25.0)[0] / a["dphi_inf"][0] - 1) < 1e-12
+    got = tomo.host_structure_function(np.array([1e-3]), 0.15, 1e7)[0]
+    assert abs(got / (6.8839 * (1e-3 / 0.15) ** (5.0 / 3.0)) - 1) < 1e-3
+
+
+@pytest.mark.parametrize("n,nv,nvp", [(8, 52, 69), (16, 208, 241), (20, 316, 357), (32, 812, 877), (64, 3228, 3357),
+                                       (74, 4304, 4453)])
+def test_valid_counts(n, nv, nvp):
+    """Centre-in-pupil / corner rule (Fig.2, reading G12): the counts of the configs ("~52", "~4300")."""
+    sz = tomo.host_sizes(sweep_config(n))
+    assert (sz["n_vs"], sz["n_vphi"]) == (nv, nvp)
+
+
+def test_sizes_of_the_configs():
+    assert tomo.host_sizes(get_config("cfg1"), 16, 16) == dict(n_vs=52, n_vphi=69, n_prime=9, P=16, P_os=16, Kp=1)
+    s2 = tomo.host_sizes(get_config("cfg2"))
+    assert (s2["n_prime"], s2["P"], s2["P_os"], s2["Kp"]) == (27, 40, 48, 7)
+    s3 = tomo.host_sizes(get_config("cfg3"))          # automatic: next even 5-smooth size >= 2n-1 = 147
+    assert (s3["n_prime"], s3["P"], s3["P_os"], s3["Kp"]) == (105, 150, 180, 35)
+    c3 = get_config("cfg3")                            # BASELINE.json fixes the pad of cfg3 at 160
+    assert tomo.host_sizes(c3, c3.pad, c3.pad_os)["P"] == 160
+    assert [tomo.host_sizes(sweep_config(n))["P"] for n in (16, 32, 64, 96, 128)] == [32, 64, 128, 192, 256]
+    assert [tomo.host_sizes(sweep_config(n))["P_os"] for n in (16, 32, 64, 96, 128)] == [40, 80, 160, 240, 320]
+    assert [tomo.host_sizes(sweep_config(n))["n_prime"] for n in (16, 32, 64, 96, 128)] == [25, 47, 91, 135, 179]
+
+
+@pytest.mark.parametrize("model", [tomo.TOMO_HUDGIN, tomo.TOMO_FRIED])
+@pytest.mark.parametrize("name", ["cfg1", "small_lgs"])
+def test_generators_match_oracle(name, model):
+    cfg = get_config("cfg1") if name == "cfg1" else small_lgs_config(n=9, n_gs=3, n_layers=3, targets=((5.0, -3.0),))
+    mname = "hudgin" if model == tomo.TOMO_HUDGIN else "fried"
+    dirs = [(w.ax, w.ay) for w in cfg.wfs]
+    hgs = cfg.wfs[0].h_gs
+    N, n = len(dirs), cfg.n
+    th = tz.css_generators(n, cfg.d, dirs, hgs, cfg.h, cfg.frac, cfg.r0, cfg.L0, mname).reshape(2 * N, 2 * N, 2 * n - 1, 2 * n - 1)
+    g = tomo.host_css_generators(cfg, model)
+    assert np.abs(g - th).max() <= 1e-11 * np.abs(th).max()
+    sz = tomo.host_sizes(cfg)
+    xi = tz.cos_generators(n, sz["n_prime"], cfg.d, dirs, hgs, cfg.targets[0], cfg.h, cfg.frac, cfg.r0, cfg.L0, mname)
+    if math.isinf(hgs):
+        xi = xi.sum(axis=0, keepdims=True)        # NGS: layers share one grid and are summed (Eq.15)
+    xi = xi.reshape(xi.shape[0], 2 * N, xi.shape[-1], xi.shape[-1])
+    g2 = tomo.host_cos_generators(cfg, 0, model)
+    assert g2.shape == xi.shape
+    assert np.abs(g2 - xi).max() <= 1e-11 * np.abs(xi).max()
+
+
+@pytest.mark.parametrize("P", [16, 20, 30, 48])
+def test_generator_spectrum_is_the_scaled_rfft2_of_the_embedding(P):
+    rng = np.random.default_rng(5)
+    n_in, n_out = 7, 9
+    g = rng.standard_normal((n_in + n_out - 1, n_in + n_out - 1))
+    sp = tomo.host_generator_spectrum(g, n_out, n_in, P)
+    ref = np.fft.rfft2(tz.embed_generator(g, n_in, n_out, P)) / P ** 2      # [ky][kx]
+    np.testing.assert_allclose(sp, ref.T, atol=1e-14 * np.abs(ref).max() * P)
