@@ -1,0 +1,300 @@
+#!/usr/bin/env python
+"""bench.py -- headline measurement of the hot path.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config cfg3] [--batch 1]
+
+A "step" is one pass of the whole hot path (rows A1-A8: rhs projection, n_iter CG iterations, target projection)
+over one batch of seeded synthetic slope frames.  Prints ONE JSON line (see DESIGN.md for every key).
+Multi-GPU = independent replicas of the plan: frames are dealt to ranks, no data-path collective.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "us per CG iteration & reconstructions/s at 74x74x6LGS; % of HBM/L2 roofline"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="cfg3")
+    ap.add_argument("--batch", type=int, default=1)
+    ap.add_argument("--n-iter", type=int, default=0, help="CG iterations per solve (0 = the config's count)")
+    ap.add_argument("--solver", default=os.environ.get("TOMO_SOLVER", "multikernel"), choices=["multikernel", "persistent"])
+    ap.add_argument("--precision", default="f32", choices=["f32", "f32s_f64a", "f64"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+# ------------------------------------------------------------------------------------------------ clocks
+class ClockSampler:
+    """Samples SM clock and throttle reasons with NVML while the timed regions run."""
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._t = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        names = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20,
+                 "hw_power_brake_slowdown": 0x80, "sync_boost": 0x10}
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            time.sleep(0.02)
+
+    def start(self):
+        if self.nv is not None:
+            self._t = threading.Thread(target=self._run, daemon=True)
+            self._t.start()
+
+    def stop(self):
+        self._stop.set()
+        if self._t is not None:
+            self._t.join()
+        return {"sm_mhz": statistics.median(self.samples) if self.samples else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# ------------------------------------------------------------------------------------------------ reference arm
+def oracle_setup(cfg, n_iter):
+    """The fp64 oracle, as it stands, on a bounded sample of the workload.  Returns (step, description, cores);
+    step() runs the sample once and returns the seconds per reconstruction it implies.
+    ELT sizes: ONE full matrix-free direct-sum Sigma_ss product (oracle/directsum.c, OpenMP) is timed and multiplied
+    by n_iter (the target projection is left out); tiny/mid sizes: the dense oracle's full CG solve + projection."""
+    import numpy as np
+    from oracle import directsum
+    from oracle import toeplitz as tz
+    from oracle.system import OracleSystem
+    cores = len(os.sched_getaffinity(0))
+    if 2 * cfg.n_wfs * cfg.n * cfg.n <= 6000:
+        from tomo_inputs import screens
+        osys = OracleSystem(cfg)
+        s = screens.generate(cfg, osys.sigma2)["slopes"].ravel()
+
+        def step():
+            t0 = time.perf_counter()
+            x, _ = osys.solve_cg(s, n_iter)
+            osys.reconstruct(x, 0)
+            return time.perf_counter() - t0
+        return step, f"dense fp64 oracle: full {n_iter}-iteration CG solve + projection", cores
+    osys = OracleSystem(cfg, dense=False)
+    # the direct sum's cost does not depend on the generator values: only the rows of WFS 0 are built (the oracle's
+    # numpy generator build takes minutes for all N^2 pairs); the product itself is timed in full
+    theta = tz.css_generators(cfg.n, cfg.d, osys.dirs, osys.h_gs, cfg.h, cfg.frac, cfg.r0, cfg.L0, wfs_rows=[0])
+    v = np.random.default_rng(1).standard_normal(osys.Ns)
+    directsum.css_mvm(theta, osys.ix, osys.iy, v)
+
+    def step():
+        t0 = time.perf_counter()
+        directsum.css_mvm(theta, osys.ix, osys.iy, v)
+        return (time.perf_counter() - t0) * n_iter
+    return step, (f"matrix-free fp64 oracle (oracle/directsum.c, OpenMP): one full direct-sum Sigma_ss product timed, "
+                  f"x{n_iter} iterations; target projection not included"), cores
+
+
+def run_reference(args, cfg, n_iter, rank):
+    if rank != 0:
+        return
+    step, desc, cores = oracle_setup(cfg, n_iter)
+    for _ in range(min(max(args.warmup, 0), 2)):
+        step()
+    k = max(1, min(args.steps, 5))
+    sec = statistics.mean(step() for _ in range(k))
+    val = 1.0 / sec
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": "reconstructions/s", "n_gpus": args.gpus,
+            "steps": k, "warmup": min(max(args.warmup, 0), 2), "ms_per_step": sec * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg.name, "batch": 1, "n_iter": n_iter},
+            "us_per_cg_iteration": sec / n_iter * 1e6,
+            "cpu_baseline": {"value": val, "unit": "reconstructions/s", "cores": cores, "kind": "oracle", "sample": desc},
+            "e2e": {"value": val, "unit": "reconstructions/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------------ our arm
+def main():
+    args = parse()
+    from tomo_inputs.configs import get_config
+    cfg = get_config(args.config)
+    n_iter = args.n_iter or cfg.n_iter
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, cfg, n_iter, rank)
+        return
+
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_1806_07938_b200 import tomo
+    from paper_1806_07938_b200.replicas import barrier, max_over_ranks
+    from tomo_inputs import screens
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the library has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    prec = {"f32": tomo.TOMO_F32, "f32s_f64a": tomo.TOMO_F32S_F64A, "f64": tomo.TOMO_F64}[args.precision]
+    solver = tomo.TOMO_SOLVER_PERSISTENT if args.solver == "persistent" else tomo.TOMO_SOLVER_MULTIKERNEL
+    B = args.batch
+    t0 = time.perf_counter()
+    plan = tomo.TomoPlan(cfg, max_batch=B, precision=prec, solver=solver)
+    t_plan = time.perf_counter() - t0
+    sigma2 = float(plan.noise()[0][0])
+    # every rank (replica) gets its own frames: seed offset by rank
+    data = screens.generate(cfg, sigma2, n_frames=B, seed_offset=10 * rank)
+    h_slopes = torch.from_numpy(np.ascontiguousarray(data["slopes"].reshape(B, -1), dtype=np.float32)).pin_memory()
+    d_slopes = h_slopes.cuda()
+    d_out = torch.empty(B * plan.wavefront_len, dtype=torch.float32, device="cuda")
+    stream = torch.cuda.current_stream()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
+
+    def timed(n_it, steps, do_flush=True):
+        """device time of `steps` solves, each bracketed by its own CUDA events (the L2 flush is outside)."""
+        evs = []
+        for _ in range(steps):
+            if do_flush:
+                flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            plan.solve_batch(d_slopes, d_out, B, n_it, stream=stream)
+            b.record(stream)
+            evs.append((a, b))
+        torch.cuda.synchronize()
+        return sum(a.elapsed_time(b) for a, b in evs)
+
+    for _ in range(max(args.warmup, 3)):
+        plan.solve_batch(d_slopes, d_out, B, n_iter, stream=stream)
+        plan.solve_batch(d_slopes, d_out, B, 0, stream=stream)
+    torch.cuda.synchronize()
+    launches = plan.stats()["launches_last_solve"]
+    plan.solve_batch(d_slopes, d_out, B, n_iter, stream=stream)
+    launches = plan.stats()["launches_last_solve"]
+
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    barrier(world)
+    torch.cuda.synchronize()
+    ms_total = timed(n_iter, args.steps)                # THE timed region: exactly K steps
+    torch.cuda.synchronize()
+    barrier(world)
+    ms_total = max_over_ranks(ms_total, world)
+    ms_step = ms_total / args.steps
+    k0 = max(3, min(args.steps, 50))
+    ms_step0 = max_over_ranks(timed(0, k0), world) / k0             # A1 + A7-A8 only -> per-iteration time by difference
+    # L2-warm steady state (what a real-time loop sees: nothing else touches the GPU between frames)
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(stream)
+    for _ in range(args.steps):
+        plan.solve_batch(d_slopes, d_out, B, n_iter, stream=stream)
+    b.record(stream)
+    torch.cuda.synchronize()
+    ms_step_warm = max_over_ranks(a.elapsed_time(b), world) / args.steps
+    # end to end through the public API with HOST buffers: pinned H2D + solve + D2H, synchronised per step
+    e2e = []
+    for i in range(args.steps + 3):
+        flush.zero_()
+        torch.cuda.synchronize()
+        t1 = time.perf_counter()
+        out_h = plan.solve_host(h_slopes, n_iter, n_frames=B, stream=stream)
+        stream.synchronize()
+        e2e.append(time.perf_counter() - t1)
+    e2e_ms = max_over_ranks(statistics.mean(e2e[3:]) * 1e3, world)
+    clocks = sampler.stop()
+
+    # per-kernel device times of the multi-kernel loop (CUDA events after every kernel, on the launch stream)
+    kt = plan.time_kernels(B, n_iter, stream=stream) if args.solver == "multikernel" else None
+    n, C, P = cfg.n, 2 * cfg.n_wfs, plan.P
+    Ph, Ns, npair = P // 2 + 1, 2 * cfg.n_wfs * plan.n_vs, C * (C + 1) // 2
+    E = 4 if prec == tomo.TOMO_F32 else 8
+    SE = 8 if prec == tomo.TOMO_F64 else 4
+    spectra = npair * P * Ph * 2 * SE
+    tbuf = C * Ph * n * 2 * E
+    kbytes = {"cols": spectra + B * 2 * tbuf, "rows_fwd": B * (3 * Ns * E + tbuf), "rows_inv": B * (tbuf + 3 * Ns * E),
+              "update": B * 6 * Ns * E}
+    b_iter = spectra + B * 9 * Ns * E
+    hbm, how = peaks()
+    us_iter = (ms_step - ms_step0) / n_iter * 1e3
+    roof = None
+    if kt:
+        dom = max(kt, key=kt.get)
+        ach = kbytes[dom] / (kt[dom] * 1e-3) / 1e9
+        roof = {"kernel": "k_" + dom, "bound": "hbm", "achieved": ach, "peak": hbm, "unit": "GB/s", "frac": ach / hbm,
+                "traffic": None, "peak_source": how, "algorithmic_bytes_per_launch": kbytes[dom],
+                "us_per_launch": {k: v * 1e3 for k, v in kt.items()},
+                "state": "in situ inside the iteration loop (spectra L2-resident after the first iteration)"}
+    iter_roof = {"b_iter_bytes": b_iter, "us_per_iteration": us_iter, "achieved_GBps": b_iter / (us_iter * 1e-6) / 1e9,
+                 "frac_of_hbm_peak": b_iter / (us_iter * 1e-6) / 1e9 / hbm}
+
+    value = world * B * 1e3 / ms_step
+    line = {"metric": METRIC, "value": value, "unit": "reconstructions/s", "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": args.precision, "data": "synthetic",
+            "config": {"workload": cfg.name, "n": cfg.n, "n_wfs": cfg.n_wfs, "n_layers": cfg.n_layers, "pad": plan.P,
+                       "pad_os": plan.P_os, "n_iter": n_iter, "batch": B, "targets": len(cfg.targets),
+                       "solver": args.solver, "parallelism": f"replicas x{world}",
+                       "l2": "flushed (256 MiB write) before every timed step"},
+            "us_per_cg_iteration": us_iter, "ms_per_step_n_iter0": ms_step0, "ms_per_step_l2_warm": ms_step_warm,
+            "reconstructions_per_s_l2_warm": world * B * 1e3 / ms_step_warm,
+            "iteration_roofline": iter_roof, "roofline": roof,
+            "e2e": {"value": world * B * 1e3 / e2e_ms, "unit": "reconstructions/s", "ms_per_step": e2e_ms,
+                    "h2d_bytes_per_step": int(h_slopes.numel() * 4), "d2h_bytes_per_step": int(out_h.numel() * 4)},
+            "gpu_launches": launches * args.steps, "launches_per_step": launches, "clocks": clocks,
+            "plan_build_s": t_plan, "device_bytes": plan.stats()["device_bytes"]}
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        step, desc, cores = oracle_setup(cfg, n_iter)
+        sec = statistics.mean(step() for _ in range(3))
+        line["cpu_baseline"] = {"value": 1.0 / sec, "unit": "reconstructions/s", "cores": cores, "kind": "oracle",
+                                "sample": desc, "us_per_cg_iteration": sec / n_iter * 1e6}
+    if rank == 0:
+        print(json.dumps(line))
+    plan.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

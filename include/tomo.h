@@ -130,6 +130,12 @@ int tomo_cg_step(tomo_plan *plan, float *x, float *r, float *p, double *rho_alph
 /* The CG solution zeta of the last solve: device->device copy into zeta_out (device fp32 [n_frames][C][n_vs]). */
 int tomo_get_zeta(tomo_plan *plan, float *zeta_out, int n_frames, void *cuda_stream);
 
+/* Measurement aid (bench.py "roofline"): runs n_iter iterations of the multi-kernel loop (A2-A6) on the state the
+ * last solve left in the plan, un-graphed, with a CUDA event after every kernel on `cuda_stream`, synchronises the
+ * stream and returns the mean device time per launch in ms: ms_out (host fp32 [4]) = rows_fwd, cols, rows_inv,
+ * update.  The state of the last solve is overwritten. */
+int tomo_time_kernels(tomo_plan *plan, int n_frames, int n_iter, float *ms_out, void *cuda_stream);
+
 /* Sizes fixed at plan creation; any pointer may be NULL. */
 int tomo_get_sizes(const tomo_plan *plan, int *n_vs, int *n_vphi, int *slopes_len, int *wavefront_len,
                    int *pad, int *pad_os, int *n_prime);

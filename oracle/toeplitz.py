@@ -95,8 +95,9 @@ def rbt_mvm_fft2(theta, x_img, n_out, P):
 
 
 # ----------------------------------------------------------------------------- generators
-def css_generators(n, d, wfs_dirs, h_gs, h, frac, r0, L0, model="hudgin"):
-    """theta[i, a, j, b, ly+(n-1), lx+(n-1)]  (L150, L265)."""
+def css_generators(n, d, wfs_dirs, h_gs, h, frac, r0, L0, model="hudgin", wfs_rows=None):
+    """theta[i, a, j, b, ly+(n-1), lx+(n-1)]  (L150, L265).  wfs_rows: compute only the output WFSs i listed
+    (the others stay zero) -- used to time a bounded sample of the ELT-size product; arithmetic unchanged."""
     N = len(wfs_dirs)
     L = 2 * n - 1
     lag = np.arange(-(n - 1), n)
@@ -106,7 +107,7 @@ def css_generators(n, d, wfs_dirs, h_gs, h, frac, r0, L0, model="hudgin"):
     th = np.zeros((N, 2, N, 2, L, L))
     for hk, fk in zip(h, frac):
         g = cone_factor(hk, h_gs)
-        for i in range(N):
+        for i in (range(N) if wfs_rows is None else wfs_rows):
             for j in range(N):
                 sh = hk * (np.asarray(wfs_dirs[j]) - np.asarray(wfs_dirs[i])) * ARCSEC
                 delta = g * d * lagv + sh

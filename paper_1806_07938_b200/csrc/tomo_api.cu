@@ -261,6 +261,14 @@ static int grid_for(int items, int per_cta) { return std::max(1, std::min((items
         if (e_ != cudaSuccess) { set_error(std::string("kernel launch: ") + cudaGetErrorString(e_)); return TOMO_ECUDA; } \
     } while (0)
 
+static inline void prof_mark(tomo_plan *pl, cudaStream_t st) {
+    if (!pl->prof) return;
+    cudaEvent_t e;
+    cudaEventCreate(&e);
+    cudaEventRecord(e, st);
+    pl->prof->push_back(e);
+}
+
 template <typename T, typename S> struct Ops {
     typedef typename cx_of<T>::type C2;
     typedef typename cx_of<S>::type S2;
@@ -290,19 +298,23 @@ template <typename T, typename S> struct Ops {
         a.partials_r = pl->d_partials_r; a.n_part = n_part; a.part_stride = pl->part_stride;
         a.hist = pl->d_hist; a.alpha = pl->d_alpha;
         const int items = F * m.C * pl->g.npairs;
+        prof_mark(pl, st);
         k_rows_fwd<T><<<grid_for(items, kRowWarps), 32 * kRowWarps, rows_smem<T>(m.P), st>>>(a);
         LAUNCH_CHECK();
+        prof_mark(pl, st);
         ColsArgs<T, S> c;
         c.st = a.st; c.g = pl->g; c.T1 = (const C2 *)pl->d_T1; c.T2 = (C2 *)pl->d_T2;
         c.spec = (const S2 *)pl->d_spec; c.n_pair = m.n_pair;
         const int nw = cols_warps(m.C);
         k_cols<T, S><<<dim3(m.Ph, F), 32 * nw, cols_smem<T>(m.P, m.C, nw), st>>>(c);
         LAUNCH_CHECK();
+        prof_mark(pl, st);
         RowsInvArgs<T> b;
         b.st = a.st; b.g = pl->g; b.F = F; b.T2 = (const C2 *)pl->d_T2; b.p = (const T *)pl->d_p;
         b.sigma2 = (const T *)pl->d_sigma2; b.q = (T *)pl->d_q; b.partials_q = pl->d_partials_q;
         k_rows_inv<T><<<grid_for(items, kRowWarps), 32 * kRowWarps, rows_smem<T>(m.P), st>>>(b);
         LAUNCH_CHECK();
+        prof_mark(pl, st);
         pl->launches_last += 3;
         return TOMO_OK;
     }
@@ -361,6 +373,7 @@ template <typename T, typename S> struct Ops {
             if ((rc = mvm(pl, st, F, k > 0, 1, k, k == 0 ? n_part0 : pl->upd_blocks))) return rc;
             k_update<T><<<dim3(pl->upd_blocks, F), 256, 0, st>>>(update_args(pl, k));
             LAUNCH_CHECK();
+            prof_mark(pl, st);
             pl->launches_last += 1;
         }
         k_finalize<<<F, 32, 0, st>>>(pl->d_partials_r, n_iter == 0 ? n_part0 : pl->upd_blocks, pl->part_stride,
@@ -495,6 +508,29 @@ template <typename T, typename S> struct Ops {
         return TOMO_OK;
     }
 
+    // one un-graphed pass of the iteration loop on the plan-held state with an event after every kernel
+    static int time_kernels(tomo_plan *pl, int F, int n_iter, float *ms_out, cudaStream_t st) {
+        int rc;
+        if ((rc = prepare(pl))) return rc;
+        std::vector<cudaEvent_t> ev;
+        pl->prof = &ev;
+        rc = enqueue_loop(pl, st, F, n_iter, pl->upd_blocks, false);
+        pl->prof = nullptr;
+        cudaError_t e = cudaStreamSynchronize(st);
+        double acc[4] = {0, 0, 0, 0};
+        if (!rc && e == cudaSuccess && (int)ev.size() == 5 * n_iter)
+            for (int k = 0; k < n_iter; ++k)
+                for (int j = 0; j < 4; ++j) {
+                    float ms = 0.f;
+                    cudaEventElapsedTime(&ms, ev[5 * k + j], ev[5 * k + j + 1]);
+                    acc[j] += ms;
+                }
+        else if (!rc) { set_error("profiling pass failed"); rc = TOMO_ECUDA; }
+        for (cudaEvent_t x : ev) cudaEventDestroy(x);
+        for (int j = 0; j < 4; ++j) ms_out[j] = (float)(acc[j] / std::max(n_iter, 1));
+        return rc;
+    }
+
     static int get_zeta(tomo_plan *pl, float *out, int F, cudaStream_t st) {
         const size_t cnt = (size_t)F * pl->m.C * pl->m.nv;
         k_convert<T, float><<<(unsigned)std::min<size_t>((cnt + 255) / 256, 148 * 8), 256, 0, st>>>((const T *)pl->d_x, out, cnt);
@@ -563,6 +599,13 @@ extern "C" int tomo_get_zeta(tomo_plan *pl, float *zeta_out, int n_frames, void 
     if (rc) return rc;
     if (!zeta_out || n_frames < 1 || n_frames > pl->F) { set_error("bad arguments"); return TOMO_EINVAL; }
     return DISPATCH(pl, get_zeta(pl, zeta_out, n_frames, (cudaStream_t)cuda_stream));
+}
+
+extern "C" int tomo_time_kernels(tomo_plan *pl, int n_frames, int n_iter, float *ms_out, void *cuda_stream) {
+    int rc = check_ready(pl);
+    if (rc) return rc;
+    if (!ms_out || n_frames < 1 || n_frames > pl->F || n_iter < 1 || n_iter >= pl->hist_cap) { set_error("bad arguments"); return TOMO_EINVAL; }
+    return DISPATCH(pl, time_kernels(pl, n_frames, n_iter, ms_out, (cudaStream_t)cuda_stream));
 }
 
 extern "C" int tomo_get_sizes(const tomo_plan *pl, int *n_vs, int *n_vphi, int *slopes_len, int *wavefront_len,

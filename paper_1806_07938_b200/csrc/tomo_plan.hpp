@@ -45,6 +45,7 @@ struct tomo_plan {
     // graph cache: (n_frames, n_iter, warm) -> executable graph of the iteration loop + projection
     std::map<std::tuple<int, int, int>, cudaGraphExec_t> graphs;
     std::map<std::tuple<int, int, int>, int> graph_launches;   // kernel nodes in each cached graph
+    std::vector<cudaEvent_t> *prof = nullptr;   // when set, launch sequences bracket every kernel with events
     void *persist = nullptr;     // persistent-solver state (solve_persistent.cu)
 };
 

@@ -23,7 +23,7 @@ TOMO_SOLVER_MULTIKERNEL, TOMO_SOLVER_PERSISTENT = 0, 1
 
 EXPORTS = (
     "tomo_plan_create", "tomo_plan_upload_kernels", "tomo_solve", "tomo_solve_batch", "tomo_apply_css",
-    "tomo_apply_cos", "tomo_cg_step", "tomo_get_zeta", "tomo_get_sizes", "tomo_get_valid_index", "tomo_get_noise",
+    "tomo_apply_cos", "tomo_cg_step", "tomo_get_zeta", "tomo_time_kernels", "tomo_get_sizes", "tomo_get_valid_index", "tomo_get_noise",
     "tomo_get_residuals", "tomo_get_stats", "tomo_plan_destroy", "tomo_last_error",
     "tomo_host_sizes", "tomo_host_css_generators", "tomo_host_cos_generators", "tomo_host_generator_spectrum",
     "tomo_host_structure_function",
@@ -87,6 +87,7 @@ def load(build_if_missing: bool = True):
     lib.tomo_apply_cos.argtypes = [vp, fp, fp, vp]
     lib.tomo_cg_step.argtypes = [vp, fp, fp, fp, vp, vp]
     lib.tomo_get_zeta.argtypes = [vp, fp, C.c_int, vp]
+    lib.tomo_time_kernels.argtypes = [vp, C.c_int, C.c_int, C.POINTER(C.c_float), vp]
     lib.tomo_get_sizes.argtypes = [vp, ip, ip, ip, ip, ip, ip, ip]
     lib.tomo_get_valid_index.argtypes = [vp, ip, ip]
     lib.tomo_get_noise.argtypes = [vp, dp, dp]
@@ -244,6 +245,11 @@ class TomoPlan:
 
     def get_zeta(self, zeta_out, n_frames: int = 1, stream=None):
         _check(self.lib.tomo_get_zeta(self._h, _ptr(zeta_out), n_frames, _stream_handle(stream)))
+
+    def time_kernels(self, n_frames: int, n_iter: int, stream=None):
+        ms = (C.c_float * 4)()
+        _check(self.lib.tomo_time_kernels(self._h, n_frames, n_iter, ms, _stream_handle(stream)))
+        return dict(zip(("rows_fwd", "cols", "rows_inv", "update"), [float(v) for v in ms]))
 
     # -- getters --
     def valid_index(self):
