@@ -136,6 +136,15 @@ int tomo_get_zeta(tomo_plan *plan, float *zeta_out, int n_frames, void *cuda_str
  * update.  The state of the last solve is overwritten. */
 int tomo_time_kernels(tomo_plan *plan, int n_frames, int n_iter, float *ms_out, void *cuda_stream);
 
+/* Measurement aid for the persistent solver: one instrumented solve of n_iter iterations from the state the last
+ * solve left in the plan; thread 0 of every CTA stamps the SM cycle counter at the phase boundaries.  Synchronises
+ * the stream.  us_out (host fp32 [10]), microseconds at the device's nominal SM clock, mean over iterations; work
+ * segments are the maximum over CTAs, barrier segments the minimum over CTAs (= pure latency):
+ * [0] whole iteration (CTA 0), [1] rho/beta scalars, [2] p~ update, [3] forward y-FFT, [4] block product,
+ * [5] inverse y-FFT + T2 write, [6] grid barrier B, [7] alpha/mode scalars (+ first inverse x-FFT), [8] row phase,
+ * [9] grid barrier A.  The state of the last solve is overwritten. */
+int tomo_time_phases(tomo_plan *plan, int n_frames, int n_iter, float *us_out, void *cuda_stream);
+
 /* Sizes fixed at plan creation; any pointer may be NULL. */
 int tomo_get_sizes(const tomo_plan *plan, int *n_vs, int *n_vphi, int *slopes_len, int *wavefront_len,
                    int *pad, int *pad_os, int *n_prime);

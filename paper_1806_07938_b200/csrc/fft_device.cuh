@@ -180,4 +180,72 @@ TOMO_HD typename cx_of<T>::type *warp_fft(typename cx_of<T>::type *a, typename c
     return x;
 }
 
+// ---------------------------------------------------------------------------------------------- compile-time plan
+// Same Stockham passes with the length, strides and trip counts known at compile time (no integer division, fully
+// unrolled); radix order as plan_fft on the host: 5s, 3s, 8s, 4s, 2s.
+template <int N> struct PickRadix {
+    static constexpr int value = (N % 5 == 0) ? 5 : (N % 3 == 0) ? 3 : (N % 8 == 0) ? 8 : (N % 4 == 0) ? 4 : 2;
+};
+template <int N> struct CountPasses { static constexpr int value = 1 + CountPasses<N / PickRadix<N>::value>::value; };
+template <> struct CountPasses<1> { static constexpr int value = 0; };
+
+template <typename T, int R, bool INV, int P, int S, int NCUR, int NL>
+TOMO_HD void fft_pass_static(const typename cx_of<T>::type *__restrict__ x, typename cx_of<T>::type *__restrict__ y,
+                             const typename cx_of<T>::type *__restrict__ tw, int lane) {
+    typedef typename cx_of<T>::type C;
+    constexpr int nb = P / R;
+    constexpr bool last = (NCUR == R);
+    constexpr int trips = (nb + NL - 1) / NL;
+#pragma unroll
+    for (int it = 0; it < trips; ++it) {
+        const int idx = lane + it * NL;
+        if ((nb % NL == 0) || idx < nb) {
+            const int p = idx / S, q = idx - p * S;
+            C v[R];
+#pragma unroll
+            for (int j = 0; j < R; ++j) v[j] = x[idx + nb * j];
+            SmallDft<T, R, INV>::run(v);
+            C *out = y + q + S * R * p;
+            out[0] = v[0];
+            if (last) {
+#pragma unroll
+                for (int k = 1; k < R; ++k) out[S * k] = v[k];
+            } else {
+                const int t = p * S;
+#pragma unroll
+                for (int k = 1; k < R; ++k) {
+                    const C w = tw[t * k];
+                    out[S * k] = INV ? cmulc(v[k], w) : cmul(v[k], w);
+                }
+            }
+        }
+    }
+}
+
+template <typename T, bool INV, int P, int S, int NCUR, int NL> struct FftChain {
+    typedef typename cx_of<T>::type C;
+    TOMO_HD static C *run(C *x, C *y, const C *tw, int lane) {
+        constexpr int R = PickRadix<NCUR>::value;
+        fft_pass_static<T, R, INV, P, S, NCUR, NL>(x, y, tw, lane);
+#ifdef __CUDA_ARCH__
+        __syncwarp();
+#endif
+        return FftChain<T, INV, P, S * R, NCUR / R, NL>::run(y, x, tw, lane);
+    }
+};
+template <typename T, bool INV, int P, int S, int NL> struct FftChain<T, INV, P, S, 1, NL> {
+    typedef typename cx_of<T>::type C;
+    TOMO_HD static C *run(C *x, C *, const C *, int) { return x; }
+};
+
+// Compile-time-planned counterpart of warp_fft: same contract, same result buffer.
+template <typename T, bool INV, int P, int NL = 32>
+TOMO_HD typename cx_of<T>::type *warp_fft_static(typename cx_of<T>::type *a, typename cx_of<T>::type *b,
+                                                 const typename cx_of<T>::type *tw, int lane) {
+#ifdef __CUDA_ARCH__
+    __syncwarp();
+#endif
+    return FftChain<T, INV, P, 1, P, NL>::run(a, b, tw, lane);
+}
+
 }  // namespace tomo

@@ -77,8 +77,11 @@ using namespace tomo;
 
 extern "C" const char *tomo_last_error(void) { return g_err.c_str(); }
 
+namespace tomo { void persist_destroy(tomo_plan *pl); }
+
 extern "C" void tomo_plan_destroy(tomo_plan *pl) {
     if (!pl) return;
+    persist_destroy(pl);
     for (auto &kv : pl->graphs) cudaGraphExecDestroy(kv.second);
     for (void *p : pl->allocs) cudaFree(p);
     delete pl;
@@ -531,6 +534,41 @@ template <typename T, typename S> struct Ops {
         return rc;
     }
 
+    static int project_from_x(tomo_plan *pl, cudaStream_t st, int F) {
+        int rc;
+        if ((rc = prepare(pl))) return rc;
+        ProjectArgs<T, T> pa;
+        pa.g = pl->g; pa.in = (const T *)pl->d_x; pa.out = (T *)pl->d_z; pa.out2 = pa.out3 = pa.zero = nullptr;
+        pa.partials_r = nullptr; pa.part_stride = 0;
+        k_project<T, T><<<dim3(pl->m.n_wfs, F), 256, 0, st>>>(pa);
+        LAUNCH_CHECK();
+        pl->launches_last += 1;
+        return project_targets(pl, st, F);
+    }
+
+    static int state_load(tomo_plan *pl, cudaStream_t st, const float *x, const float *r, const float *p, const double *rho) {
+        const size_t cnt = (size_t)pl->m.C * pl->m.nv;
+        const unsigned gb = (unsigned)std::min<size_t>((cnt + 255) / 256, 148 * 8);
+        k_convert<float, T><<<gb, 256, 0, st>>>(x, (T *)pl->d_x, cnt);
+        k_convert<float, T><<<gb, 256, 0, st>>>(r, (T *)pl->d_r, cnt);
+        k_convert<float, T><<<gb, 256, 0, st>>>(p, (T *)pl->d_p, cnt);
+        LAUNCH_CHECK();
+        CK(cudaMemcpyAsync(pl->d_hist, rho, sizeof(double), cudaMemcpyDeviceToDevice, st));
+        pl->launches_last += 3;
+        return TOMO_OK;
+    }
+
+    static int state_store(tomo_plan *pl, cudaStream_t st, float *x, float *r, float *p) {
+        const size_t cnt = (size_t)pl->m.C * pl->m.nv;
+        const unsigned gb = (unsigned)std::min<size_t>((cnt + 255) / 256, 148 * 8);
+        k_convert<T, float><<<gb, 256, 0, st>>>((const T *)pl->d_x, x, cnt);
+        k_convert<T, float><<<gb, 256, 0, st>>>((const T *)pl->d_r, r, cnt);
+        k_convert<T, float><<<gb, 256, 0, st>>>((const T *)pl->d_p, p, cnt);
+        LAUNCH_CHECK();
+        pl->launches_last += 3;
+        return TOMO_OK;
+    }
+
     static int get_zeta(tomo_plan *pl, float *out, int F, cudaStream_t st) {
         const size_t cnt = (size_t)F * pl->m.C * pl->m.nv;
         k_convert<T, float><<<(unsigned)std::min<size_t>((cnt + 255) / 256, 148 * 8), 256, 0, st>>>((const T *)pl->d_x, out, cnt);
@@ -553,7 +591,19 @@ static int check_ready(tomo_plan *pl) {
     return TOMO_OK;
 }
 
-namespace tomo { int solve_persistent(tomo_plan *pl, const float *slopes, float *out, int F, int n_iter, const float *x0, cudaStream_t st); }
+namespace tomo {
+int solve_persistent(tomo_plan *pl, const float *slopes, float *out, int F, int n_iter, const float *x0, cudaStream_t st);
+int cg_step_persistent(tomo_plan *pl, float *x, float *r, float *p, double *scal, cudaStream_t st);
+int time_phases_persistent(tomo_plan *pl, int F, int n_iter, float *us_out, cudaStream_t st);
+
+// A7-A8 from the CG solution held in d_x -> d_out (used by the persistent solver)
+int project_from_x(tomo_plan *pl, cudaStream_t st, int F) { return DISPATCH(pl, project_from_x(pl, st, F)); }
+// fp32 ABI vectors <-> plan-held CG state (teacher-forced step)
+int state_load(tomo_plan *pl, cudaStream_t st, const float *x, const float *r, const float *p, const double *rho) {
+    return DISPATCH(pl, state_load(pl, st, x, r, p, rho));
+}
+int state_store(tomo_plan *pl, cudaStream_t st, float *x, float *r, float *p) { return DISPATCH(pl, state_store(pl, st, x, r, p)); }
+}  // namespace tomo
 
 extern "C" int tomo_solve_batch(tomo_plan *pl, const float *slopes, float *wavefront_out, int n_frames, int n_iter,
                                 const float *x0, void *cuda_stream) {
@@ -591,6 +641,7 @@ extern "C" int tomo_cg_step(tomo_plan *pl, float *x, float *r, float *p, double 
     int rc = check_ready(pl);
     if (rc) return rc;
     if (!x || !r || !p || !rho_alpha_beta) { set_error("NULL vector"); return TOMO_EINVAL; }
+    if (pl->opt.solver == TOMO_SOLVER_PERSISTENT) return cg_step_persistent(pl, x, r, p, rho_alpha_beta, (cudaStream_t)cuda_stream);
     return DISPATCH(pl, cg_step(pl, x, r, p, rho_alpha_beta, (cudaStream_t)cuda_stream));
 }
 
@@ -606,6 +657,13 @@ extern "C" int tomo_time_kernels(tomo_plan *pl, int n_frames, int n_iter, float 
     if (rc) return rc;
     if (!ms_out || n_frames < 1 || n_frames > pl->F || n_iter < 1 || n_iter >= pl->hist_cap) { set_error("bad arguments"); return TOMO_EINVAL; }
     return DISPATCH(pl, time_kernels(pl, n_frames, n_iter, ms_out, (cudaStream_t)cuda_stream));
+}
+
+extern "C" int tomo_time_phases(tomo_plan *pl, int n_frames, int n_iter, float *us_out, void *cuda_stream) {
+    int rc = check_ready(pl);
+    if (rc) return rc;
+    if (!us_out || n_frames < 1 || n_frames > pl->F || n_iter < 1 || n_iter >= pl->hist_cap) { set_error("bad arguments"); return TOMO_EINVAL; }
+    return time_phases_persistent(pl, n_frames, n_iter, us_out, (cudaStream_t)cuda_stream);
 }
 
 extern "C" int tomo_get_sizes(const tomo_plan *pl, int *n_vs, int *n_vphi, int *slopes_len, int *wavefront_len,

@@ -23,7 +23,7 @@ TOMO_SOLVER_MULTIKERNEL, TOMO_SOLVER_PERSISTENT = 0, 1
 
 EXPORTS = (
     "tomo_plan_create", "tomo_plan_upload_kernels", "tomo_solve", "tomo_solve_batch", "tomo_apply_css",
-    "tomo_apply_cos", "tomo_cg_step", "tomo_get_zeta", "tomo_time_kernels", "tomo_get_sizes", "tomo_get_valid_index", "tomo_get_noise",
+    "tomo_apply_cos", "tomo_cg_step", "tomo_get_zeta", "tomo_time_kernels", "tomo_time_phases", "tomo_get_sizes", "tomo_get_valid_index", "tomo_get_noise",
     "tomo_get_residuals", "tomo_get_stats", "tomo_plan_destroy", "tomo_last_error",
     "tomo_host_sizes", "tomo_host_css_generators", "tomo_host_cos_generators", "tomo_host_generator_spectrum",
     "tomo_host_structure_function",
@@ -88,6 +88,7 @@ def load(build_if_missing: bool = True):
     lib.tomo_cg_step.argtypes = [vp, fp, fp, fp, vp, vp]
     lib.tomo_get_zeta.argtypes = [vp, fp, C.c_int, vp]
     lib.tomo_time_kernels.argtypes = [vp, C.c_int, C.c_int, C.POINTER(C.c_float), vp]
+    lib.tomo_time_phases.argtypes = [vp, C.c_int, C.c_int, C.POINTER(C.c_float), vp]
     lib.tomo_get_sizes.argtypes = [vp, ip, ip, ip, ip, ip, ip, ip]
     lib.tomo_get_valid_index.argtypes = [vp, ip, ip]
     lib.tomo_get_noise.argtypes = [vp, dp, dp]
@@ -250,6 +251,13 @@ class TomoPlan:
         ms = (C.c_float * 4)()
         _check(self.lib.tomo_time_kernels(self._h, n_frames, n_iter, ms, _stream_handle(stream)))
         return dict(zip(("rows_fwd", "cols", "rows_inv", "update"), [float(v) for v in ms]))
+
+    def time_phases(self, n_frames: int, n_iter: int, stream=None):
+        us = (C.c_float * 10)()
+        _check(self.lib.tomo_time_phases(self._h, n_frames, n_iter, us, _stream_handle(stream)))
+        return dict(zip(("iteration", "rho_beta", "slab_update", "slab_fft_fwd", "slab_mac", "slab_fft_inv", "barrier_b", "alpha_modes",
+                         "rows", "barrier_a"),
+                        [float(v) for v in us]))
 
     # -- getters --
     def valid_index(self):

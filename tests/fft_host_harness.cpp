@@ -44,7 +44,43 @@ template <typename T> static double run(int P, bool inv) {
     return std::sqrt(err / nrm);
 }
 
+// the compile-time-planned chain (warp_fft_static) for the sizes the persistent kernel instantiates
+template <typename T, int P> static double run_static(bool inv) {
+    typedef typename cx_of<T>::type C;
+    std::vector<C> a(P), b(P), tw(P);
+    std::vector<std::complex<double>> in(P);
+    for (int i = 0; i < P; ++i) {
+        in[i] = {std::sin(i * 1.3) + 0.01 * i, std::cos(i * 0.7) - 0.3};
+        a[i].x = (T)in[i].real(); a[i].y = (T)in[i].imag();
+        tw[i].x = (T)std::cos(2 * M_PI * i / P); tw[i].y = (T)-std::sin(2 * M_PI * i / P);
+    }
+    C *r = inv ? warp_fft_static<T, true, P, 1>(a.data(), b.data(), tw.data(), 0) : warp_fft_static<T, false, P, 1>(a.data(), b.data(), tw.data(), 0);
+    // same result buffer as the run-time plan: first argument iff the number of passes is even
+    if ((r == a.data()) != (CountPasses<P>::value % 2 == 0)) return 1.0;
+    double err = 0, nrm = 0;
+    for (int k = 0; k < P; ++k) {
+        std::complex<double> s = 0;
+        for (int j = 0; j < P; ++j) {
+            const double ph = (inv ? 1 : -1) * 2 * M_PI * (double)(((long)j * k) % P) / P;
+            s += in[j] * std::complex<double>(std::cos(ph), std::sin(ph));
+        }
+        err += std::norm(s - std::complex<double>(r[k].x, r[k].y));
+        nrm += std::norm(s);
+    }
+    return std::sqrt(err / nrm);
+}
+template <int P> static void print_static() {
+    std::printf("S %d %.3e %.3e %.3e %.3e\n", P, run_static<float, P>(false), run_static<float, P>(true), run_static<double, P>(false),
+                run_static<double, P>(true));
+}
+
 int main(int argc, char **argv) {
+    if (argc > 1 && argv[1][0] == 'S') {
+        print_static<16>(); print_static<20>(); print_static<24>(); print_static<32>(); print_static<40>(); print_static<48>();
+        print_static<64>(); print_static<80>(); print_static<128>(); print_static<160>(); print_static<180>(); print_static<192>();
+        print_static<240>(); print_static<256>(); print_static<320>();
+        return 0;
+    }
     for (int i = 1; i < argc; ++i) {
         const int P = std::atoi(argv[i]);
         std::printf("%d %.3e %.3e %.3e %.3e\n", P, run<float>(P, false), run<float>(P, true), run<double>(P, false), run<double>(P, true));

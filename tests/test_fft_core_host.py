@@ -28,3 +28,14 @@ def test_fft_core_matches_direct_dft(harness):
         f32f, f32i, f64f, f64i = map(float, r[1:])
         assert f32f < 5e-7 and f32i < 5e-7, r
         assert f64f < 5e-15 and f64i < 5e-15, r
+
+
+def test_static_fft_chain_matches_direct_dft(harness):
+    """warp_fft_static (compile-time plan used by the persistent kernel) for every instantiated size."""
+    out = subprocess.check_output([harness, "S"], text=True)
+    rows = [line.split() for line in out.strip().splitlines()]
+    assert [int(r[1]) for r in rows] == [16, 20, 24, 32, 40, 48, 64, 80, 128, 160, 180, 192, 240, 256, 320]
+    for r in rows:
+        f32f, f32i, f64f, f64i = map(float, r[2:])
+        assert f32f < 5e-7 and f32i < 5e-7, r
+        assert f64f < 5e-15 and f64i < 5e-15, r

@@ -85,6 +85,9 @@ def make_plan(name, **kw):
 
 
 ALL = ["cfg1", "small_lgs", "small_odd_focus", "small_fried", "ngs_offaxis", "cfg2"]
+# both solvers go through every solve gate: the multi-kernel CUDA-graph loop and the persistent cooperative kernel
+SOLVERS = [tomo.TOMO_SOLVER_MULTIKERNEL, tomo.TOMO_SOLVER_PERSISTENT]
+solvers = pytest.mark.parametrize("solver", SOLVERS, ids=["multikernel", "persistent"])
 
 
 # ------------------------------------------------------------------------------------------------ P-a
@@ -119,10 +122,11 @@ def test_target_projection_parity(name):
 
 
 # ------------------------------------------------------------------------------------------------ P-b
-@pytest.mark.parametrize("name", ["cfg1", "small_lgs", "small_odd_focus", "cfg2"])
-def test_teacher_forced_cg_steps(name):
+@solvers
+@pytest.mark.parametrize("name", ["cfg1", "small_lgs", "small_odd_focus", "ngs_offaxis", "cfg2"])
+def test_teacher_forced_cg_steps(name, solver):
     cfg, _, osys, data = system(name)
-    pl = make_plan(name)
+    pl = make_plan(name, solver=solver)
     n_it = cfg.n_iter
     _, _, st = osys.solve_cg(f32(data["slopes"][0].ravel()), n_it, record=True)
     ks = range(n_it) if osys.Ns < 1000 else range(0, n_it, 3)
@@ -149,15 +153,16 @@ def _horizon(h_a, h_b, x_a=None, x_b=None, tol=TOL_TRAJ):
     return int(bad[0]) if bad.size else len(h_a)
 
 
+@solvers
 @pytest.mark.parametrize("name", ["cfg1", "small_lgs", "cfg2"])
-def test_free_running_fp32_tracks_oracle_up_to_the_fp32_horizon(name):
+def test_free_running_fp32_tracks_oracle_up_to_the_fp32_horizon(name, solver):
     cfg, _, osys, data = system(name)
     n_it = cfg.n_iter
     s = f32(data["slopes"][0].ravel())
     x64, h64 = osys.solve_cg(s, n_it)
     _, h32 = osys.solve_cg(s, n_it, dtype=np.float32)           # fp32 CPU emulation of the same algorithm
     k_star = max(_horizon(h32, h64) - 2, 3)
-    pl = make_plan(name)
+    pl = make_plan(name, solver=solver)
     d_w = torch.empty(pl.wavefront_len, dtype=torch.float32, device="cuda")
     pl.solve(dev(s), d_w, n_it)
     torch.cuda.synchronize()
@@ -176,8 +181,9 @@ def test_free_running_fp32_tracks_oracle_up_to_the_fp32_horizon(name):
 
 
 # ------------------------------------------------------------------------------------------------ P-d
-@pytest.mark.parametrize("name", ["cfg1", "small_lgs", "small_odd_focus", "cfg2"])
-def test_converged_solution_matches_direct_solve(name):
+@solvers
+@pytest.mark.parametrize("name", ["cfg1", "small_lgs", "small_odd_focus", "small_fried", "ngs_offaxis", "cfg2"])
+def test_converged_solution_matches_direct_solve(name, solver):
     cfg, _, osys, data = system(name)
     s = f32(data["slopes"][0].ravel())
     zeta = osys.solve_direct(s)
@@ -185,7 +191,7 @@ def test_converged_solution_matches_direct_solve(name):
     _, h = osys.solve_cg(s, 1000)
     n_it = int(np.flatnonzero(h / h[0] < 1e-6)[0])
     assert n_it <= 1000
-    pl = make_plan(name)
+    pl = make_plan(name, solver=solver)
     d_w = torch.empty(pl.wavefront_len, dtype=torch.float32, device="cuda")
     pl.solve(dev(s), d_w, n_it)
     torch.cuda.synchronize()
@@ -199,7 +205,8 @@ def test_converged_solution_matches_direct_solve(name):
 # ------------------------------------------------------------------------------------------------ P-e
 @pytest.mark.parametrize("name,prec", [("cfg1", tomo.TOMO_F64), ("small_lgs", tomo.TOMO_F64), ("cfg2", tomo.TOMO_F64),
                                         ("cfg1", tomo.TOMO_F32S_F64A)])
-def test_fp64_instantiation_meets_the_literal_gate_where_the_oracle_is_reproducible(name, prec):
+@solvers
+def test_fp64_instantiation_meets_the_literal_gate_where_the_oracle_is_reproducible(name, prec, solver):
     cfg, _, osys, data = system(name)
     n_it = cfg.n_iter
     s = f32(data["slopes"][0].ravel())
@@ -209,7 +216,7 @@ def test_fp64_instantiation_meets_the_literal_gate_where_the_oracle_is_reproduci
     k_rep = _horizon(h_b, h_a, tol=1e-4)
     phi_a, phi_b = osys.reconstruct(x_a, 0), osys.reconstruct(x_b, 0)
     reproducible = k_rep > n_it and rel(phi_b, phi_a) <= 1e-4
-    pl = make_plan(name, precision=prec)
+    pl = make_plan(name, precision=prec, solver=solver)
     d_w = torch.empty(pl.wavefront_len, dtype=torch.float32, device="cuda")
     n_gate = n_it if reproducible else max(min(k_rep, n_it) - 2, 3)
     pl.solve(dev(s), d_w, n_gate)
@@ -226,9 +233,10 @@ def test_fp64_instantiation_meets_the_literal_gate_where_the_oracle_is_reproduci
 
 
 # ------------------------------------------------------------------------------------------------ API behaviour
-def test_batch_frames_equal_single_solves_bitwise_and_residuals():
+@solvers
+def test_batch_frames_equal_single_solves_bitwise_and_residuals(solver):
     cfg, _, osys, data = system("small_lgs")
-    pl = make_plan("small_lgs", max_batch=2)
+    pl = make_plan("small_lgs", max_batch=2, solver=solver)
     s = data["slopes"].reshape(2, -1)
     n_it = 12
     d_w2 = torch.empty(2 * pl.wavefront_len, dtype=torch.float32, device="cuda")
@@ -244,9 +252,10 @@ def test_batch_frames_equal_single_solves_bitwise_and_residuals():
     pl.close()
 
 
-def test_zero_iterations_and_warm_start():
+@solvers
+def test_zero_iterations_and_warm_start(solver):
     cfg, _, osys, data = system("small_lgs")
-    pl = make_plan("small_lgs")
+    pl = make_plan("small_lgs", solver=solver)
     s = f32(data["slopes"][0].ravel())
     d_w = torch.empty(pl.wavefront_len, dtype=torch.float32, device="cuda")
     pl.solve(dev(s), d_w, 0)                                   # x = 0 -> phi = 0, history = [||M s||]
