@@ -16,7 +16,9 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtomo_b200.so")
 OBJ = os.path.join(HERE, "build")
 
-CU = ["tomo_api.cu", "solve_persistent.cu"]
+PERSIST_SIZES = [16, 20, 24, 32, 40, 64, 128, 160, 192, 256]     # TOMO_PERSIST_SIZES in csrc/persist_host.cuh
+CU = [("tomo_api.cu", "tomo_api", []), ("solve_persistent.cu", "solve_persistent", [])] + \
+     [("persist_inst.cu", f"persist_inst_{p}", [f"-DTOMO_PINST={p}"]) for p in PERSIST_SIZES]
 CPP = ["host_model.cpp", "host_kernels.cpp"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC,-fopenmp", "-I", os.path.join(ROOT, "include"), "-I", CSRC]
@@ -42,20 +44,30 @@ def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(OBJ, exist_ok=True)
     objs = []
     procs = []
-    for f in CU:
-        o = os.path.join(OBJ, f + ".o")
-        cmd = [nvcc, *NVCC_FLAGS, "-c", os.path.join(CSRC, f), "-o", o]
+    jobs = []
+    for f, stem, extra in CU:
+        o = os.path.join(OBJ, stem + ".o")
+        cmd = [nvcc, *NVCC_FLAGS, *extra, "-c", os.path.join(CSRC, f), "-o", o]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
-        procs.append((cmd, subprocess.Popen(cmd)))
+        jobs.append(cmd)
         objs.append(o)
     for f in CPP:
         o = os.path.join(OBJ, f + ".o")
-        cmd = ["g++", *CXX_FLAGS, "-c", os.path.join(CSRC, f), "-o", o]
-        procs.append((cmd, subprocess.Popen(cmd)))
+        jobs.append(["g++", *CXX_FLAGS, "-c", os.path.join(CSRC, f), "-o", o])
         objs.append(o)
-    for cmd, p in procs:
+    # at most one compiler per core at a time
+    width = max(1, min(len(jobs), os.cpu_count() or 4))
+    running = []
+    pending = list(jobs)
+    while pending or running:
+        while pending and len(running) < width:
+            cmd = pending.pop(0)
+            running.append((cmd, subprocess.Popen(cmd)))
+        cmd, p = running.pop(0)
         if p.wait() != 0:
+            for _, q in running:
+                q.kill()
             raise RuntimeError("build failed: " + " ".join(cmd))
     subprocess.check_call([nvcc, "-shared", "-o", LIB, *objs, "-Xcompiler", "-fopenmp", "-lgomp",
                            "-gencode", "arch=compute_100a,code=sm_100a"])

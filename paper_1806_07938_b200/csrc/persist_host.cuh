@@ -1,0 +1,86 @@
+// persist_host.cuh -- host side of the persistent solver shared by solve_persistent.cu (prepare, dispatch) and the
+// per-size translation units persist_inst.cu (kernel instantiation + launch).
+#pragma once
+#include <algorithm>
+#include <cstring>
+#include <string>
+
+#include "tomo.h"
+#include "persist_kernel.cuh"
+#include "tomo_plan.hpp"
+
+namespace tomo {
+
+// FFT edges the persistent kernel is instantiated for (one translation unit each); other sizes use the multi-kernel solver
+#define TOMO_PERSIST_SIZES(X) X(16) X(20) X(24) X(32) X(40) X(64) X(128) X(160) X(192) X(256)
+
+struct PersistState {
+    unsigned *d_flags = nullptr;
+    void *d_T1 = nullptr, *d_T1p = nullptr, *d_T2 = nullptr, *d_mspec = nullptr, *d_s2c = nullptr;
+    void *d_xd = nullptr, *d_rd = nullptr, *d_pd = nullptr, *d_bd = nullptr;
+    double *d_part_r = nullptr, *d_part_s = nullptr, *d_part_i = nullptr;
+    int G = 0, nq_m = 1, NQ = 0, SB = 0, any_remove = 0, spec_smem = 0, vec_smem = 0;
+    int off_ms = 0, off_work = 0, off_red = 0, off_scal = 0, off_tab = 0, off_upart = 0, off_vm = 0, off_vec = 0, off_spec = 0, off_ptab = 0, ngs = 2;
+    size_t smem = 0;
+    bool attr_set = false;
+};
+
+struct PLaunch {
+    int F, n_iter, mode, finalize_p;
+    const float *slopes, *x0;
+    double *scal_out;
+    long long *dbg;
+};
+
+#define PCK(call)                                                                 \
+    do {                                                                          \
+        cudaError_t e_ = (call);                                                  \
+        if (e_ != cudaSuccess) {                                                  \
+            set_error(std::string(#call) + ": " + cudaGetErrorString(e_));        \
+            return TOMO_ECUDA;                                                    \
+        }                                                                         \
+    } while (0)
+
+template <int P> int persist_run(tomo_plan *pl, cudaStream_t st, const PLaunch &L);
+
+template <typename T, typename S, int P>
+static int persist_launch(tomo_plan *pl, cudaStream_t st, const PLaunch &L) {
+    typedef typename cx_of<T>::type C2;
+    typedef typename cx_of<S>::type S2;
+    PersistState *ps = (PersistState *)pl->persist;
+    const HostModel &m = pl->m;
+    PArgs<T, S> a;
+    std::memset(&a, 0, sizeof(a));
+    a.g = pl->g;
+    a.P = m.P; a.Ph = m.Ph; a.tw = (const C2 *)pl->d_tw;
+    a.F = L.F; a.n_iter = L.n_iter; a.mode = L.mode; a.finalize_p = L.finalize_p;
+    a.npad = 2 * pl->g.npairs; a.U = m.C * pl->g.npairs; a.NQ = ps->NQ; a.nq_m = ps->nq_m; a.SB = ps->SB;
+    a.G = std::max(1, std::min(ps->G, std::max(L.F * a.U, m.Ph)));
+    a.spec_smem = ps->spec_smem; a.vec_smem = ps->vec_smem; a.any_remove = ps->any_remove;
+    a.off_ms = ps->off_ms; a.off_work = ps->off_work; a.off_red = ps->off_red; a.off_scal = ps->off_scal;
+    a.off_tab = ps->off_tab; a.off_upart = ps->off_upart; a.off_vm = ps->off_vm; a.off_vec = ps->off_vec;
+    a.off_spec = ps->off_spec; a.off_ptab = ps->off_ptab; a.ngs = ps->ngs;
+    a.s_in = L.slopes; a.x0 = L.x0;
+    a.x = (T *)pl->d_x; a.r = (T *)pl->d_r; a.p = (T *)pl->d_p;
+    a.xd = (T *)ps->d_xd; a.rd = (T *)ps->d_rd; a.pd = (T *)ps->d_pd; a.bd = (T *)ps->d_bd;
+    a.T1 = (C2 *)ps->d_T1; a.T1p = (C2 *)ps->d_T1p; a.T2 = (C2 *)ps->d_T2;
+    a.spec = (const S2 *)pl->d_spec; a.n_pair = m.n_pair;
+    a.mspec = (const C2 *)ps->d_mspec; a.s2c = (const T *)ps->d_s2c;
+    a.part_r = ps->d_part_r; a.part_s = ps->d_part_s; a.part_i = ps->d_part_i;
+    a.hist = pl->d_hist; a.hist_stride = pl->hist_cap; a.alpha = pl->d_alpha; a.scal_out = L.scal_out;
+    a.flags = ps->d_flags; a.dbg = L.dbg;
+    if (!ps->attr_set) {
+        PCK(cudaFuncSetAttribute((k_persistent<T, S, P>), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ps->smem));
+        int occ = 0;
+        PCK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (k_persistent<T, S, P>), kPThreads, ps->smem));
+        if (occ < 1) { set_error("persistent kernel does not fit on an SM"); return TOMO_EUNSUPPORTED; }
+        ps->attr_set = true;
+    }
+    PCK(cudaMemsetAsync(ps->d_flags, 0, 1024, st));
+    void *kargs[] = {&a};
+    PCK(cudaLaunchCooperativeKernel((const void *)(k_persistent<T, S, P>), dim3(a.G), dim3(kPThreads), kargs, ps->smem, st));
+    pl->launches_last += 1;
+    return TOMO_OK;
+}
+
+}  // namespace tomo

@@ -1,0 +1,698 @@
+// persist_kernel.cuh -- persistent cooperative CG solver: ONE kernel per solve, two grid barriers per iteration,
+// every 1-D transform held in registers (fft_reg.cuh: two passes, one shared-memory exchange).
+//
+// The textbook CG recurrences (PAPER.md S2.G L337, Eq.12) are kept, but the work is re-ordered so that an
+// iteration has only the two all-to-all exchanges the 2-D FFT itself needs:
+//
+//   phase C_k (one CTA per k_x slab, all channels):   rho_k, beta_k from the r.r partials;
+//        p~rows_k = r~rows_k + beta_k p~rows_{k-1}    (the x-FFT is linear, so p = r + beta p is formed in the
+//                                                      half-transformed domain; p~rows stays with its slab)
+//        y-FFT, per-frequency C x C block product with the Hermitian-packed kernel spectra pinned in shared
+//        memory (Eq.22, Eq.30), + sigma^2 p~ (Sigma_eta, L260), inverse y-FFT -> T2
+//        p.q and the modal sums Z^T q (Eq.36) by Parseval from p~, y~ and the mask spectra
+//   ---- grid barrier B ----
+//   phase R_k (16 lanes per (channel, row pair)):      alpha_k = rho_k / p.q, mode coefficients;
+//        inverse x-FFT, crop + mask (S_2, W_s; Eq.24-27, Eq.34), q' = M_s q,
+//        p_k = r_k + beta_k p_{k-1} (spatial copy), x += alpha p, r -= alpha q', partial r.r,
+//        forward x-FFT of the NEW residual rows (S_1, Eq.18-21) -> T1
+//   ---- grid barrier A ----
+//
+// p.q is taken in the frequency domain (Parseval; p is zero outside the pupil, so the crop does not matter and
+// p.M_s q = p.q for p in range(M_s)); every reduction is a fixed-order sum with fp64 scalars, so a fixed-count
+// solve is bit-reproducible.  Sigma_eta must be uniform per channel here (all configs).
+//
+// Every 1-D transform is the same two shared-memory-to-shared-memory passes (P = A * B, A <= B <= 16; fft_reg.cuh):
+//   pass 1  thread j2 < B:  radix A over j = j1 B + j2, twiddle W_P^{j2 k1}  -> Y[k1 (B+1) + j2]
+//   pass 2  thread k1 < A:  radix B over j2                                  -> X[k1 + A k2]
+// done by TWO small non-inlined codelets that the slab phase, the row phase, the forward and the inverse transforms
+// all share (an inverse transform is the forward one on conjugated data: conj on the way in, conj on the way out).
+// The whole per-iteration instruction footprint has to stay within the 32 KB L1.5 instruction cache: the first
+// register-FFT version of this kernel was fully unrolled (333 KB of SASS) and stalled on instruction fetch.
+#pragma once
+#include <cuda_runtime.h>
+
+#include "fft_reg.cuh"
+#include "tomo_kernels.cuh"
+
+namespace tomo {
+
+static const int kPThreads = 512;
+static const int kPWarps = kPThreads / 32;
+static const int kGS = 16;                       // lanes per row unit
+
+enum { PM_COLD = 0, PM_WARM = 1, PM_STATE = 2 };
+enum { PT_START = 0, PT_RHO = 1, PT_BUILD = 2, PT_FFT = 3, PT_MAC = 4, PT_INV = 5, PT_BAR_B = 6, PT_SCAL = 7, PT_ROWS = 8, PT_BAR_A = 9, PT_R_LOAD = 10, PT_R_FFT1 = 11, PT_R_UPD = 12, PT_R_FFT2 = 13, PT_N = 16 };
+
+// per-frame scalar block in shared memory (doubles)
+enum { SC_RHO = 0, SC_RHO_PREV = 1, SC_BETA = 2, SC_ALPHA = 3, SC_UPD = 4, SC_PQ = 5, SC_HEAD = 6 };
+
+template <typename T, typename S> struct PArgs {
+    DevGeom g;
+    int P, Ph;
+    const typename cx_of<T>::type *tw;   // device [P], exp(-2 pi i t/P)
+    int F, n_iter, mode, finalize_p;
+    int G;                       // grid size (CTAs)
+    int npad;                    // 2 * npairs
+    int U;                       // row units per frame = C * npairs
+    int NQ;                      // slab partial quantities: 1 + C (+ C with focus removal)
+    int nq_m;                    // mask spectra: 1 (mask) or 3 (mask, x-weighted, y-weighted)
+    int SB;                      // doubles per frame in the scalar block
+    int spec_smem;               // kernel spectra slice pinned in shared memory
+    int vec_smem;                // x, r, p rows of the CTA's units held in shared memory for the whole solve
+    int any_remove;
+    // shared-memory layout (byte offsets)
+    int off_ms, off_work, off_red, off_scal, off_tab, off_upart, off_vm, off_vec, off_spec, off_ptab;
+    int ngs;                     // row-unit buffer slots in shared memory = row units processed per round
+    const float *s_in;           // [F][C][nv] slopes (COLD/WARM)
+    const float *x0;             // [F][C][nv] warm start (WARM)
+    T *x, *r, *p;                // [F][C][nv] valid-only layout (ABI side)
+    T *xd, *rd, *pd, *bd;        // [F][C][npad][n] dense rows (solver side; xd/rd/pd unused with vec_smem)
+    typename cx_of<T>::type *T1;    // [F][Ph][C][npad]     x-FFT of the current residual rows
+    typename cx_of<T>::type *T1p;   // [F][Ph][C][npad]     x-FFT of the search direction (slab-private state)
+    typename cx_of<T>::type *T2;    // [F][C][npairs][Ph][2]
+    const typename cx_of<S>::type *spec;   // [Ph][n_pair][P]
+    int n_pair;
+    const typename cx_of<T>::type *mspec;  // [nq_m][Ph][P]  spectra of the pupil mask (and coordinate-weighted masks)
+    const T *s2c;                // [C] sigma^2_c / P^2
+    double *part_r;              // [F][G]       r.r per CTA
+    double *part_s;              // [F][NQ][Ph]  per slab: p.q, sum q_c, sum coord q_c
+    double *part_i;              // [F][U][2]    init: sum s, sum coord s per row unit
+    double *hist;                // [F][hist_stride] rho_k
+    int hist_stride;
+    double *alpha;               // [F]
+    double *scal_out;            // [3] rho_{k+1}, alpha, beta (finalize_p, frame 0) or NULL
+    unsigned *flags;             // arrival counter of the grid barrier
+    long long *dbg;              // [G][n_iter][PT_N] clock64 stamps of thread 0 (measurement aid) or NULL
+};
+
+// ---- grid barrier: one arrival counter.  Writers: data stores -> bar.sync -> thread 0: red.release.
+// Readers: thread 0 ld.acquire until all arrived -> bar.sync -> L2 (.cg) loads of the exchanged data.
+__device__ __forceinline__ void grid_sync(unsigned *ctr, unsigned target) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(ctr) : "memory");
+        unsigned v;
+        do {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(ctr) : "memory");
+        } while ((int)(v - target) < 0);
+    }
+    __syncthreads();
+}
+
+template <typename T> __device__ __forceinline__ double div_as(double a, double b) { return (double)((T)a / (T)b); }
+
+// sum over the 16 lanes of a row-unit group (every lane of the group returns the total)
+__device__ __forceinline__ double group_sum(double v) {
+#pragma unroll
+    for (int o = kGS / 2; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// deterministic sum by one warp of up to 160 contiguous doubles other CTAs wrote: all loads in flight at once
+__device__ __forceinline__ double warp_sum_cg160(const double *src, int count, int lane) {
+    double v[5];
+#pragma unroll
+    for (int m = 0; m < 5; ++m) { const int i = lane + 32 * m; v[m] = (i < count) ? __ldcg(src + i) : 0.0; }
+    return warp_sum(((v[0] + v[1]) + (v[2] + v[3])) + v[4]);
+}
+__device__ __forceinline__ double warp_sum_cg(const double *src, int count, int stride, int lane) {
+    double s = 0.0;
+    for (int i = lane; i < count; i += 32) s += __ldcg(src + (size_t)i * stride);
+    return warp_sum(s);
+}
+
+// two adjacent complex values (16-byte aligned for fp32) through L2
+__device__ __forceinline__ void ldcg_pair(const float2 *p, float2 &u, float2 &v) {
+    const float4 t = __ldcg(reinterpret_cast<const float4 *>(p));
+    u = make_float2(t.x, t.y); v = make_float2(t.z, t.w);
+}
+__device__ __forceinline__ void ldcg_pair(const double2 *p, double2 &u, double2 &v) { u = __ldcg(p); v = __ldcg(p + 1); }
+__device__ __forceinline__ void st_pair(float2 *p, float2 u, float2 v) { *reinterpret_cast<float4 *>(p) = make_float4(u.x, u.y, v.x, v.y); }
+__device__ __forceinline__ void st_pair(double2 *p, double2 u, double2 v) { p[0] = u; p[1] = v; }
+__device__ __forceinline__ float2 shfl_c(float2 v, int src) {
+    return make_float2(__shfl_sync(0xffffffffu, v.x, src), __shfl_sync(0xffffffffu, v.y, src));
+}
+__device__ __forceinline__ double2 shfl_c(double2 v, int src) {
+    return make_double2(__shfl_sync(0xffffffffu, v.x, src), __shfl_sync(0xffffffffu, v.y, src));
+}
+
+// ---- the two codelets: R-point DFT from src (stride ss) to dst (stride ds), optional twiddle tw[tj * k]
+template <typename T, int R, bool TW>
+__device__ __noinline__ void dft_pass(const typename cx_of<T>::type *src, int ss, typename cx_of<T>::type *dst, int ds,
+                                      const typename cx_of<T>::type *tw, int tj) {
+    typedef typename cx_of<T>::type C2;
+    C2 v[R];
+#pragma unroll
+    for (int j = 0; j < R; ++j) v[j] = src[j * ss];
+    SmallDft<T, R, false>::run(v);
+    dst[0] = v[0];
+#pragma unroll
+    for (int k = 1; k < R; ++k) dst[k * ds] = TW ? cmul(v[k], tw[tj * k]) : v[k];
+}
+
+struct PairRef { int off; float sgn; };          // spectrum block of (c_out, c_in): element offset and conjugation sign
+
+// ---- per-frequency block product of one k_x slab (Eq.22, Eq.30) + Sigma_eta (L260) + Parseval partials.
+// Warps are grouped: WPG = ceil(P/32) warps cover the k_y range, group g owns a contiguous range of output channels.
+// X: forward y-spectra [c][LD] in natural k_y order; Y: [c][LD], CONJUGATED (the inverse transform is run as a forward
+// one).  CT > 0: the C inputs of this k_y are held in registers; CT = 0: run-time channel count.
+// red: [Goc][P] partial p.q, then [C][P] mask sums, then [C][P] focus sums.
+template <typename T, typename S, int CT>
+__device__ __forceinline__ void mac_slab(const typename cx_of<T>::type *X, typename cx_of<T>::type *Y, int LD,
+                                         const typename cx_of<S>::type *spec, const PairRef *ptab,
+                                         const typename cx_of<T>::type *ms, const T *s2c,
+                                         int C, int P, int nq_m, int any_remove, T *red, int warp, int lane) {
+    typedef typename cx_of<T>::type C2;
+    typedef typename cx_of<S>::type S2;
+    const int WPG = (P + 31) >> 5;
+    const int Goc = min(kPWarps / WPG, C);
+    const int grp = warp / WPG, ky = (warp - grp * WPG) * 32 + lane;
+    if (grp >= Goc || ky >= P) return;
+    const int oc_lo = grp * C / Goc, oc_hi = (grp + 1) * C / Goc;
+    C2 m0 = mk<T>((T)0, (T)0), m1 = m0, m2 = m0;
+    if (any_remove) { m0 = ms[ky]; if (nq_m > 1) { m1 = ms[P + ky]; m2 = ms[2 * P + ky]; } }
+    T *red_s = red + Goc * P, *red_f = red_s + C * P;
+    const S2 *sp = spec + ky;
+    C2 x[CT > 0 ? CT : 1];
+    if (CT > 0) {
+#pragma unroll
+        for (int ci = 0; ci < CT; ++ci) x[ci] = X[ci * LD + ky];
+    }
+    T pap = (T)0;
+#pragma unroll 1
+    for (int oc = oc_lo; oc < oc_hi; ++oc) {
+        const C2 xo = X[oc * LD + ky];
+        const T s2 = s2c[oc];
+        const PairRef *row = ptab + oc * C;
+        T ar = s2 * xo.x, ai = s2 * xo.y;
+        if (CT > 0) {
+#pragma unroll
+            for (int ci = 0; ci < CT; ++ci) {
+                const PairRef e = row[ci];
+                const S2 s = sp[e.off];
+                const T sr = (T)s.x, si = (T)s.y * (T)e.sgn;
+                ar += sr * x[ci].x - si * x[ci].y;
+                ai += sr * x[ci].y + si * x[ci].x;
+            }
+        } else {
+            for (int ci = 0; ci < C; ++ci) {
+                const PairRef e = row[ci];
+                const S2 s = sp[e.off];
+                const C2 xv = X[ci * LD + ky];
+                const T sr = (T)s.x, si = (T)s.y * (T)e.sgn;
+                ar += sr * xv.x - si * xv.y;
+                ai += sr * xv.y + si * xv.x;
+            }
+        }
+        Y[oc * LD + ky] = mk<T>(ar, -ai);
+        pap += xo.x * ar + xo.y * ai;                               // Re(conj(p~) y~)
+        if (any_remove) {
+            red_s[oc * P + ky] = m0.x * ar + m0.y * ai;             // Re(conj(m~) y~)
+            if (nq_m > 1) { const C2 mm = (oc & 1) ? m2 : m1; red_f[oc * P + ky] = mm.x * ar + mm.y * ai; }
+        }
+    }
+    red[grp * P + ky] = pap;
+}
+
+// fixed-order sum of `cnt` values of the slab partial array by one warp
+template <typename T> __device__ __forceinline__ double warp_sum_red(const T *src, int cnt, int lane) {
+    T s = (T)0;
+    for (int i = lane; i < cnt; i += 32) s += src[i];
+    return warp_sum((double)s);
+}
+
+template <typename T, typename S, int P>
+__global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
+    typedef typename cx_of<T>::type C2;
+    typedef typename cx_of<S>::type S2;
+    constexpr int A = Fact2<P>::A, B = Fact2<P>::B, Ph = P / 2 + 1;
+    constexpr int LD = A * (B + 1);               // row stride of the slab buffers and size of a pass-1 result
+    static_assert(A * B == P && A >= 2 && A <= B && B <= kGS, "unsupported split");
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int n = a.g.n, nv = a.g.nv, C = a.g.C, npairs = a.g.npairs, N = a.g.N;
+    const int F = a.F, U = a.U, NQ = a.NQ, SB = a.SB, G = a.G, npad = a.npad;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, NW = kPWarps, b = blockIdx.x;
+    const int gl = lane & (kGS - 1), gs = tid / kGS;      // lane within the row-unit group, group slot
+    C2 *tw = reinterpret_cast<C2 *>(smem_raw);
+    C2 *ms = reinterpret_cast<C2 *>(smem_raw + a.off_ms);
+    C2 *work = reinterpret_cast<C2 *>(smem_raw + a.off_work);
+    T *red = reinterpret_cast<T *>(smem_raw + a.off_red);
+    double *scal = reinterpret_cast<double *>(smem_raw + a.off_scal);
+    double *sGs = reinterpret_cast<double *>(smem_raw + a.off_tab);
+    int *s_nrem = reinterpret_cast<int *>(sGs + 9 * N);
+    T *s_s2c = reinterpret_cast<T *>(s_nrem + N + (N & 1));
+    double *upart = reinterpret_cast<double *>(smem_raw + a.off_upart);
+    unsigned *s_vm = reinterpret_cast<unsigned *>(smem_raw + a.off_vm);
+    T *svec = reinterpret_cast<T *>(smem_raw + a.off_vec);
+    S2 *sspec = reinterpret_cast<S2 *>(smem_raw + a.off_spec);
+    PairRef *ptab = reinterpret_cast<PairRef *>(smem_raw + a.off_ptab);
+    C2 *Ubuf = work, *Vbuf = work + (size_t)C * LD;
+    const int NGS = a.ngs;
+    C2 *bufA = work + (size_t)(gs < NGS ? gs : 0) * (P + LD), *bufB = bufA + P;   // row unit: natural [P], pass-1 result [LD]
+    unsigned epoch = 0;
+    const T half_n = (T)(0.5 * (n - 1)), dd = (T)a.g.d;
+    int k = -2;                                      // iteration index seen by PSTAMP (no stamps outside the loop)
+#define PSTAMP(pt) do { if (a.dbg && tid == 0 && k >= 0) a.dbg[((size_t)b * a.n_iter + k) * PT_N + (pt)] = clock64(); } while (0)
+#define GRID_SYNC() do { epoch += G; grid_sync(a.flags, epoch); } while (0)
+
+    // ---- slab ownership: CTA b owns k_x = b % Ph and a contiguous share of the frames
+    const int kx = b % Ph;
+    int f_lo, f_hi;
+    {
+        const int cnt = (G - 1 - kx) / Ph + 1, rk = b / Ph;
+        f_lo = (int)((long long)rk * F / cnt);
+        f_hi = (int)((long long)(rk + 1) * F / cnt);
+        if (F == 1) { f_lo = 0; f_hi = (rk == 0) ? 1 : 0; }
+    }
+    const bool has_slab = f_hi > f_lo;
+    const S2 *gspec = a.spec + (size_t)kx * a.n_pair * P;
+    const T wkx = (kx == 0 || 2 * kx == P) ? (T)1 : (T)2;
+    // slab thread maps
+    const bool it1 = tid < C * B, it2 = tid < C * A;
+    const int c1 = tid / B, j2s = tid - c1 * B;      // pass 1: (channel, j2)
+    const int c2s = tid / A, k1s = tid - c2s * A;    // pass 2: (channel, k1)
+    const int w_busy = (C * B + 31) >> 5;            // warps that carry slab pass-1 items
+    const int n_free = (NW - w_busy) > 0 ? NW - w_busy : NW;
+    // ---- row units of this CTA: ut = b + i G, i < nu; NGS of them per round, unit i0 + gs by the 16 lanes of group gs
+    const int nu = (b < F * U) ? (F * U - b + G - 1) / G : 0;
+    const int n_rounds = nu > 0 ? (nu + NGS - 1) / NGS : 1;
+
+    for (int i = tid; i < P; i += kPThreads) tw[i] = a.tw[i];
+    for (int i = tid; i < 9 * N; i += kPThreads) sGs[i] = a.g.Gs[i];
+    for (int i = tid; i < N; i += kPThreads) s_nrem[i] = a.g.n_remove[i];
+    for (int i = tid; i < C; i += kPThreads) s_s2c[i] = a.s2c[i];
+    for (int i = tid; i < C * C; i += kPThreads) {
+        const int oc = i / C, ci = i - oc * C, lo = min(oc, ci), hi = max(oc, ci);
+        PairRef e;
+        e.off = (lo * C - (lo * (lo - 1)) / 2 + hi - lo) * P;       // pair (c_out <= c_in); the transposed block is its conjugate
+        e.sgn = ci < oc ? -1.f : 1.f;
+        ptab[i] = e;
+    }
+    if (has_slab) {
+        for (int q = 0; q < a.nq_m; ++q)
+            for (int i = tid; i < P; i += kPThreads) ms[q * P + i] = a.mspec[((size_t)q * Ph + kx) * P + i];
+        if (a.spec_smem)
+            for (int i = tid; i < a.n_pair * P; i += kPThreads) sspec[i] = gspec[i];
+    }
+    for (int i = tid; i < F * SB; i += kPThreads) scal[i] = 0.0;
+    for (int i = tid; i < nu * kGS; i += kPThreads) s_vm[i] = 0u;
+    __syncthreads();
+    const S2 *spec = a.spec_smem ? sspec : gspec;
+
+    // per-WFS mode coefficients (Z^T Z)^-1 Z^T q from the channel sums (Eq.36): thread t -> (frame, WFS)
+    auto mode_coefs = [&](int t) {
+        const int f = t / N, i = t - f * N;
+        double *sc = scal + f * SB;
+        const double *S0 = sc + SC_HEAD, *S1 = sc + SC_HEAD + C;
+        const double tq[3] = {S0[2 * i], S0[2 * i + 1], S1[2 * i] + S1[2 * i + 1]};
+        const int nr = s_nrem[i];
+        for (int u = 0; u < 3; ++u) {
+            double s = 0.0;
+            if (u < nr) for (int v = 0; v < nr; ++v) s += sGs[i * 9 + u * 3 + v] * tq[v];
+            sc[SC_HEAD + 2 * C + i * 3 + u] = s;
+        }
+    };
+
+    struct Unit { int f, c, j, comp, w, y0, s0, s1, s2; bool two; size_t vbase; };
+    auto unit_of = [&](int i) {
+        Unit q;
+        const int ut = b + i * G;
+        q.f = ut / U;
+        const int u = ut - q.f * U;
+        q.c = u / npairs; q.j = u - q.c * npairs; q.comp = q.c & 1; q.w = q.c >> 1;
+        q.y0 = 2 * q.j; q.two = q.y0 + 1 < n;
+        q.s0 = a.g.row_ptr[q.y0]; q.s1 = a.g.row_ptr[q.y0 + 1]; q.s2 = a.g.row_ptr[min(q.y0 + 2, n)];
+        q.vbase = ((size_t)q.f * C + q.c) * nv;
+        return q;
+    };
+    // dense rows (2 x n) of x, r, p, b of unit i
+    auto dense = [&](int i, const Unit &q, int which) -> T * {
+        if (a.vec_smem && which < 3) return svec + ((size_t)i * 3 + which) * 2 * n;
+        T *base = which == 0 ? a.xd : which == 1 ? a.rd : which == 2 ? a.pd : a.bd;
+        return base + (((size_t)q.f * C + q.c) * npad + q.y0) * n;
+    };
+
+    // one P-point transform bufA -> bufA by the 16 lanes of a row-unit group (all 32 lanes of the warp must call)
+    auto unit_fft = [&](bool act) {
+        __syncwarp();
+        if (act && gl < B) dft_pass<T, A, true>(bufA + gl, B, bufB + gl, B + 1, tw, gl);
+        __syncwarp();
+        if (act && gl < A) dft_pass<T, B, false>(bufB + gl * (B + 1), 1, bufA + gl, A, tw, 0);
+        __syncwarp();
+    };
+    // forward x-FFT of the two rows held in bufA (.x = row y0, .y = row y0+1; zero beyond n), split into the two
+    // Hermitian half-spectra -> T1
+    auto fwd_unit = [&](const Unit &q, bool act) {
+        unit_fft(act);
+        if (act) {
+            C2 *out = a.T1 + (((size_t)q.f * Ph) * C + q.c) * npad + q.y0;
+            for (int kk = gl; kk < Ph; kk += kGS) {
+                const C2 z1 = bufA[kk], z2 = bufA[kk == 0 ? 0 : P - kk];
+                st_pair(out + (size_t)kk * C * npad, mk<T>((T)0.5 * (z1.x + z2.x), (T)0.5 * (z1.y - z2.y)),
+                        q.two ? mk<T>((T)0.5 * (z1.y + z2.y), (T)-0.5 * (z1.x - z2.x)) : mk<T>((T)0, (T)0));
+            }
+        }
+    };
+    // r.r of the CTA's units, per frame, in unit order -> part_r[f][b]
+    auto publish_rr = [&]() {
+        __syncthreads();
+        for (int f = tid; f < F; f += kPThreads) {
+            double s = 0.0;
+            for (int i = 0; i < nu; ++i) if ((b + i * G) / U == f) s += upart[i];
+            a.part_r[(size_t)f * G + b] = s;
+        }
+    };
+
+    // ================================================================ init (A1: b = M_s s, Eq.33-34)
+    // validity bits of the columns x = gl + 16 m each lane updates (bit row * 16 + m) and, for the mode removal, the
+    // per-unit sums of s
+    for (int i0 = 0; i0 < nu; i0 += NGS) {
+        const int i = i0 + gs;
+        const bool act = gs < NGS && i < nu;
+        const Unit q = unit_of(act ? i : 0);
+        double t0 = 0.0, t1 = 0.0;
+        if (act) {
+            for (int e = q.s0 + gl; e < q.s2; e += kGS) {
+                const int row = e >= q.s1, xc = a.g.ix[e];
+                atomicOr(&s_vm[i * kGS + (xc & (kGS - 1))], 1u << (row * 16 + xc / kGS));
+                if (a.any_remove && a.mode != PM_STATE) {
+                    const double v = (double)a.s_in[q.vbase + e];
+                    const double coord = ((q.comp ? q.y0 + row : xc) - 0.5 * (n - 1)) * a.g.d;
+                    t0 += v; t1 += coord * v;
+                }
+            }
+        }
+        __syncwarp();
+        if (a.any_remove && a.mode != PM_STATE) {
+            t0 = group_sum(t0); t1 = group_sum(t1);
+            if (act && gl == 0) {
+                const int u = (b + i * G) - q.f * U;
+                a.part_i[((size_t)q.f * U + u) * 2] = t0; a.part_i[((size_t)q.f * U + u) * 2 + 1] = t1;
+            }
+        }
+    }
+    if (a.any_remove && a.mode != PM_STATE) {
+        GRID_SYNC();
+        for (int item = warp; item < F * C * 2; item += NW) {
+            const int f = item / (2 * C), rem = item - f * 2 * C, e = rem / C, c = rem - e * C;
+            const double s = warp_sum_cg(a.part_i + ((size_t)f * U + c * npairs) * 2 + e, npairs, 2, lane);
+            if (lane == 0) scal[f * SB + SC_HEAD + rem] = s;
+        }
+        __syncthreads();
+        for (int t = tid; t < F * N; t += kPThreads) mode_coefs(t);
+    }
+    __syncthreads();
+    for (int i0 = 0; i0 < nu; i0 += NGS) {
+        const int i = i0 + gs;
+        const bool act = gs < NGS && i < nu;
+        const Unit q = unit_of(act ? i : 0);
+        T *ux = dense(i, q, 0), *ur = dense(i, q, 1), *up = dense(i, q, 2), *ub = dense(i, q, 3);
+        double rr = 0.0;
+        __syncwarp();
+        if (act) {
+            for (int e = gl; e < 2 * n; e += kGS) { ux[e] = (T)0; ur[e] = (T)0; up[e] = (T)0; if (a.mode == PM_WARM) ub[e] = (T)0; }
+            for (int e = gl; e < P; e += kGS) bufA[e] = mk<T>((T)0, (T)0);
+        }
+        __syncwarp();
+        if (act) {
+            const double *coef = scal + q.f * SB + SC_HEAD + 2 * C + q.w * 3;
+            for (int e = q.s0 + gl; e < q.s2; e += kGS) {
+                const int row = e >= q.s1, xc = a.g.ix[e], idx = row * n + xc;
+                T fv;                                               // first transform: p_0 = b (cold), x0 (warm), p (state)
+                if (a.mode == PM_STATE) {
+                    ux[idx] = a.x[q.vbase + e]; ur[idx] = a.r[q.vbase + e]; fv = a.p[q.vbase + e]; up[idx] = fv;
+                } else {
+                    const double coord = ((q.comp ? q.y0 + row : xc) - 0.5 * (n - 1)) * a.g.d;
+                    const T bv = (T)((double)a.s_in[q.vbase + e] - (coef[q.comp] + coef[2] * coord));   // b = s - Z a
+                    if (a.mode == PM_WARM) { ub[idx] = bv; fv = (T)a.x0[q.vbase + e]; ux[idx] = fv; }
+                    else { ur[idx] = bv; up[idx] = bv; fv = bv; rr += (double)bv * (double)bv; }         // cold: x = 0, r = p = b
+                }
+                if (row) bufA[xc].y = fv; else bufA[xc].x = fv;
+            }
+        }
+        rr = group_sum(rr);
+        if (act && gl == 0) upart[i] = rr;
+        fwd_unit(q, act);
+    }
+    publish_rr();
+    GRID_SYNC();
+
+    // ================================================================ iterations (k = -1 is the warm-start product A x0)
+    const int k_begin = (a.mode == PM_WARM) ? -1 : 0;
+    const int n_t1 = C * npairs;                        // complex pairs in one T1 slab
+#pragma unroll 1
+    for (k = k_begin; k < a.n_iter; ++k) {
+        const bool pre = k < 0;
+        const bool take_new = pre || k == 0;            // p~ = T1 (p_0, or x0 for the warm-start product)
+        PSTAMP(PT_START);
+        // ---------------------------------------------------------- phase C: slab (kx, f)
+        C2 n0[2], n1[2], o0[2], o1[2];
+        auto prefetch_slab = [&](int f, bool with_old) {
+            const C2 *t1 = a.T1 + ((size_t)f * Ph + kx) * C * npad;
+            const C2 *t1p = a.T1p + ((size_t)f * Ph + kx) * C * npad;
+#pragma unroll
+            for (int m = 0; m < 2; ++m) {
+                const int e2 = tid + m * kPThreads;
+                if (e2 < n_t1) {
+                    ldcg_pair(t1 + 2 * e2, n0[m], n1[m]);
+                    if (with_old) ldcg_pair(t1p + 2 * e2, o0[m], o1[m]);
+                }
+            }
+        };
+        if (has_slab) prefetch_slab(f_lo, !take_new);
+        // scalars: rho_k, beta_k (one warp per frame, from the top warp down)
+        if (!pre) {
+            for (int f = NW - 1 - warp; f < F; f += NW) {
+                double rho;
+                if (k == 0 && a.mode == PM_STATE) rho = a.hist[(size_t)f * a.hist_stride];
+                else rho = warp_sum_cg160(a.part_r + (size_t)f * G, G, lane);
+                if (lane == 0) {
+                    double *sc = scal + f * SB;
+                    const double rho_prev = sc[SC_RHO];
+                    const bool upd = (k > 0) && (sc[SC_ALPHA] != 0.0) && (rho_prev > 0.0);
+                    sc[SC_RHO_PREV] = rho_prev;
+                    sc[SC_RHO] = rho;
+                    sc[SC_BETA] = upd ? div_as<T>(rho, rho_prev) : 0.0;
+                    sc[SC_UPD] = upd ? 1.0 : 0.0;
+                    if (b == 0) a.hist[(size_t)f * a.hist_stride + k] = rho;
+                }
+            }
+        }
+        __syncthreads();
+        PSTAMP(PT_RHO);
+#pragma unroll 1
+        for (int f = f_lo; f < f_hi; ++f) {
+            const double *sc = scal + f * SB;
+            const bool upd = !pre && sc[SC_UPD] != 0.0;
+            const T beta = (T)sc[SC_BETA];
+            C2 *t1p = a.T1p + ((size_t)f * Ph + kx) * C * npad;
+            if (f != f_lo) prefetch_slab(f, !take_new);
+            // zero padding rows n..P-1, then p~rows = r~rows + beta p~rows_old on rows 0..n-1 -> Vbuf[c][y]
+            for (int e = tid; e < C * (P - n); e += kPThreads) { const int c = e / (P - n), y = n + e - c * (P - n); Vbuf[c * LD + y] = mk<T>((T)0, (T)0); }
+#pragma unroll
+            for (int m = 0; m < 2; ++m) {
+                const int e2 = tid + m * kPThreads;
+                if (e2 < n_t1) {
+                    C2 v0, v1;
+                    if (take_new) { v0 = n0[m]; v1 = n1[m]; }
+                    else if (upd) { v0 = mk<T>(n0[m].x + beta * o0[m].x, n0[m].y + beta * o0[m].y); v1 = mk<T>(n1[m].x + beta * o1[m].x, n1[m].y + beta * o1[m].y); }
+                    else { v0 = o0[m]; v1 = o1[m]; }
+                    if (take_new || upd) st_pair(t1p + 2 * e2, v0, v1);
+                    const int c = e2 / npairs, y = 2 * (e2 - c * npairs);
+                    Vbuf[c * LD + y] = v0;
+                    if (y + 1 < n) Vbuf[c * LD + y + 1] = v1;
+                }
+            }
+            __syncthreads();
+            PSTAMP(PT_BUILD);
+            // forward y-FFT: pass 1 Vbuf -> Ubuf, pass 2 Ubuf -> Vbuf (natural k_y)
+            if (it1) dft_pass<T, A, true>(Vbuf + c1 * LD + j2s, B, Ubuf + c1 * LD + j2s, B + 1, tw, j2s);
+            __syncthreads();
+            if (it2) dft_pass<T, B, false>(Ubuf + c2s * LD + k1s * (B + 1), 1, Vbuf + c2s * LD + k1s, A, tw, 0);
+            __syncthreads();
+            PSTAMP(PT_FFT);
+            switch (C) {
+                case 4: mac_slab<T, S, 4>(Vbuf, Ubuf, LD, spec, ptab, ms, s_s2c, C, P, a.nq_m, a.any_remove, red, warp, lane); break;
+                case 6: mac_slab<T, S, 6>(Vbuf, Ubuf, LD, spec, ptab, ms, s_s2c, C, P, a.nq_m, a.any_remove, red, warp, lane); break;
+                case 8: mac_slab<T, S, 8>(Vbuf, Ubuf, LD, spec, ptab, ms, s_s2c, C, P, a.nq_m, a.any_remove, red, warp, lane); break;
+                case 12: mac_slab<T, S, 12>(Vbuf, Ubuf, LD, spec, ptab, ms, s_s2c, C, P, a.nq_m, a.any_remove, red, warp, lane); break;
+                case 16: mac_slab<T, S, 16>(Vbuf, Ubuf, LD, spec, ptab, ms, s_s2c, C, P, a.nq_m, a.any_remove, red, warp, lane); break;
+                default: mac_slab<T, S, 0>(Vbuf, Ubuf, LD, spec, ptab, ms, s_s2c, C, P, a.nq_m, a.any_remove, red, warp, lane); break;
+            }
+            __syncthreads();
+            PSTAMP(PT_MAC);
+            // inverse y-FFT as a forward transform of conj(y~): pass 1 Ubuf -> Vbuf; the warps without pass-1 items
+            // reduce the slab partials meanwhile
+            if (it1) dft_pass<T, A, true>(Ubuf + c1 * LD + j2s, B, Vbuf + c1 * LD + j2s, B + 1, tw, j2s);
+            {
+                const int WPG = (P + 31) >> 5, Goc = min(NW / WPG, C);
+                const int slot = NW - 1 - warp;             // free warps are the top ones
+                if (slot < n_free) {
+                    for (int tq = slot; tq < NQ; tq += n_free) {
+                        double s = 0.0;
+                        if (tq == 0) s = warp_sum_red<T>(red, Goc * P, lane);
+                        else if (a.any_remove) s = warp_sum_red<T>(red + (Goc + tq - 1) * P, P, lane);
+                        if (lane == 0) a.part_s[((size_t)f * NQ + tq) * Ph + kx] = (double)wkx * s;
+                    }
+                }
+            }
+            __syncthreads();
+            if (it2) dft_pass<T, B, false>(Vbuf + c2s * LD + k1s * (B + 1), 1, Ubuf + c2s * LD + k1s, A, tw, 0);
+            __syncthreads();
+            // image rows y < n (conjugate back) -> T2[c][y / 2][kx][y & 1]
+            {
+                C2 *dst = a.T2 + (size_t)f * C * npairs * Ph * 2 + (size_t)kx * 2;
+                for (int e = tid; e < n_t1; e += kPThreads) {
+                    const int c = e / npairs, y = 2 * (e - c * npairs);
+                    const C2 u0 = Ubuf[c * LD + y], u1 = (y + 1 < n) ? Ubuf[c * LD + y + 1] : mk<T>((T)0, (T)0);
+                    st_pair(dst + (size_t)e * Ph * 2, mk<T>(u0.x, -u0.y), mk<T>(u1.x, -u1.y));
+                }
+            }
+            __syncthreads();
+        }
+        PSTAMP(PT_INV);
+        GRID_SYNC();
+        PSTAMP(PT_BAR_B);
+        // ---------------------------------------------------------- phase R: row units, NGS per round
+#pragma unroll 1
+        for (int rnd = 0; rnd < n_rounds; ++rnd) {
+            const int i = rnd * NGS + gs;
+            const bool act = gs < NGS && i < nu;
+            const Unit q = unit_of(act ? i : 0);
+            // stage 1 (no scalars needed): T2 -> conj(U + i V) with its Hermitian extension -> transform -> bufA[x] =
+            // conj(row y0 + i row y0+1) of q = A p
+            __syncwarp();
+            if (act) {
+                const C2 *src = a.T2 + (((size_t)q.f * C + q.c) * npairs + q.j) * Ph * 2;
+                constexpr int NL = (Ph + kGS - 1) / kGS;                 // all loads in flight before the first use
+                C2 u[NL], v[NL];
+#pragma unroll
+                for (int m = 0; m < NL; ++m) { const int kk = gl + m * kGS; if (kk < Ph) ldcg_pair(src + 2 * kk, u[m], v[m]); }
+#pragma unroll
+                for (int m = 0; m < NL; ++m) {
+                    const int kk = gl + m * kGS;
+                    if (kk < Ph) {
+                        bufA[kk] = mk<T>(u[m].x - v[m].y, -(u[m].y + v[m].x));                               // conj(U_k + i V_k)
+                        if (kk > 0 && 2 * kk < P) bufA[P - kk] = mk<T>(u[m].x + v[m].y, u[m].y - v[m].x);   // conj(conj(U_k) + i conj(V_k))
+                    }
+                }
+            }
+            if (rnd == 0) PSTAMP(PT_R_LOAD);
+            unit_fft(act);
+            if (rnd == 0) PSTAMP(PT_R_FFT1);
+            if (rnd == 0) {
+                // scalars: alpha_k, mode coefficients (reduction items from the top warps down)
+                for (int item = NW - 1 - warp; item < F * NQ; item += NW) {
+                    const int f = item / NQ, qq = item - f * NQ;
+                    const double s = (qq == 0 || a.any_remove) ? warp_sum_cg160(a.part_s + ((size_t)f * NQ + qq) * Ph, Ph, lane) : 0.0;
+                    if (lane == 0) scal[f * SB + (qq == 0 ? SC_PQ : SC_HEAD + qq - 1)] = s;
+                }
+                __syncthreads();
+                for (int t = tid; t < F * N; t += kPThreads) mode_coefs(t);
+                if (!pre && tid >= 32 * (NW - 1) && tid - 32 * (NW - 1) < F) {       // last warp: alpha per frame
+                    for (int f = tid - 32 * (NW - 1); f < F; f += 32) {
+                        double *sc = scal + f * SB;
+                        const double rho = sc[SC_RHO], pq = sc[SC_PQ];
+                        const double al = (rho > 0.0 && pq > 0.0) ? div_as<T>(rho, pq) : 0.0;     // breakdown: freeze (reading G16)
+                        sc[SC_ALPHA] = al;
+                        if (b == 0) a.alpha[f] = al;
+                    }
+                }
+                __syncthreads();
+                PSTAMP(PT_SCAL);
+            }
+            // stage 2: q' = M_s q, CG vector updates, r.r partial, the new residual rows -> bufA -> forward x-FFT -> T1
+            double rr = 0.0;
+            if (act) {
+                const double *sc = scal + q.f * SB;
+                const T alpha = (T)sc[SC_ALPHA], beta = (T)sc[SC_BETA];
+                const bool upd = sc[SC_UPD] != 0.0, step = sc[SC_ALPHA] != 0.0;
+                const T c0 = (T)sc[SC_HEAD + 2 * C + q.w * 3 + q.comp], c2 = (T)sc[SC_HEAD + 2 * C + q.w * 3 + 2];
+                T *ux = dense(i, q, 0), *ur = dense(i, q, 1), *up = dense(i, q, 2);
+                const T *ub = dense(i, q, 3);
+                const unsigned vm = s_vm[i * kGS + gl];
+#pragma unroll 1
+                for (int xp = gl, m = 0; xp < P; xp += kGS, ++m) {
+                    T nr[2] = {(T)0, (T)0};
+                    if (xp < n) {
+                        const C2 z = bufA[xp];
+#pragma unroll
+                        for (int row = 0; row < 2; ++row) {
+                            if ((vm >> (row * 16 + m)) & 1u) {
+                                const T coord = ((q.comp ? (T)(q.y0 + row) : (T)xp) - half_n) * dd;
+                                const T qp = (row ? -z.y : z.x) - (c0 + c2 * coord);
+                                const int idx = row * n + xp;
+                                T rv;
+                                if (pre) {                                   // warm start: r = b - M_s q, p = r
+                                    rv = ub[idx] - qp;
+                                    ur[idx] = rv; up[idx] = rv;
+                                } else {
+                                    rv = ur[idx];
+                                    T pv = up[idx];
+                                    if (upd) { pv = rv + beta * pv; up[idx] = pv; }
+                                    if (step) {
+                                        ux[idx] += alpha * pv;
+                                        rv -= alpha * qp;
+                                        ur[idx] = rv;
+                                    }
+                                }
+                                rr += (double)rv * (double)rv;
+                                nr[row] = rv;
+                            }
+                        }
+                    }
+                    bufA[xp] = mk<T>(nr[0], nr[1]);
+                }
+            }
+            rr = group_sum(rr);
+            if (act && gl == 0) upart[i] = rr;
+            if (rnd == 0) PSTAMP(PT_R_UPD);
+            fwd_unit(q, act);
+            if (rnd == 0) PSTAMP(PT_R_FFT2);
+        }
+        publish_rr();
+        PSTAMP(PT_ROWS);
+        GRID_SYNC();
+        PSTAMP(PT_BAR_A);
+    }
+    k = -2;
+
+    // ================================================================ tail: rho_{n_iter}; optional p = r + beta p; x, r, p -> valid-only layout
+    for (int f = NW - 1 - warp; f < F; f += NW) {
+        double rho;
+        if (a.n_iter == 0 && a.mode == PM_STATE) rho = a.hist[(size_t)f * a.hist_stride];
+        else rho = warp_sum_cg160(a.part_r + (size_t)f * G, G, lane);
+        if (lane == 0) {
+            double *sc = scal + f * SB;
+            const double rho_prev = sc[SC_RHO];
+            const bool upd = (a.n_iter > 0) && (sc[SC_ALPHA] != 0.0) && (rho_prev > 0.0);
+            sc[SC_BETA] = upd ? div_as<T>(rho, rho_prev) : 0.0;
+            sc[SC_UPD] = upd ? 1.0 : 0.0;
+            if (b == 0) {
+                a.hist[(size_t)f * a.hist_stride + a.n_iter] = rho;
+                if (a.scal_out && f == 0) { a.scal_out[0] = rho; a.scal_out[1] = sc[SC_ALPHA]; a.scal_out[2] = sc[SC_BETA]; }
+            }
+        }
+    }
+    __syncthreads();
+    for (int i0 = 0; i0 < nu; i0 += NGS) {
+        const int i = i0 + gs;
+        if (gs >= NGS || i >= nu) continue;
+        const Unit q = unit_of(i);
+        const double *sc = scal + q.f * SB;
+        const bool fin = a.finalize_p && sc[SC_UPD] != 0.0;
+        const T beta = (T)sc[SC_BETA];
+        const T *ux = dense(i, q, 0), *ur = dense(i, q, 1), *up = dense(i, q, 2);
+        for (int e = q.s0 + gl; e < q.s2; e += kGS) {
+            const int row = e >= q.s1, idx = row * n + a.g.ix[e];
+            T pv = up[idx];
+            const T rv = ur[idx];
+            if (fin) pv = rv + beta * pv;
+            a.x[q.vbase + e] = ux[idx]; a.r[q.vbase + e] = rv; a.p[q.vbase + e] = pv;
+        }
+    }
+#undef PSTAMP
+#undef GRID_SYNC
+}
+
+}  // namespace tomo

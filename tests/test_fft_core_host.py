@@ -39,3 +39,16 @@ def test_static_fft_chain_matches_direct_dft(harness):
         f32f, f32i, f64f, f64i = map(float, r[2:])
         assert f32f < 5e-7 and f32i < 5e-7, r
         assert f64f < 5e-15 and f64i < 5e-15, r
+
+
+def test_register_two_pass_fft_matches_direct_dft(harness):
+    """fft_reg.cuh: the two-pass register split P = A * B (both orders, forward and inverse) the persistent kernel runs."""
+    out = subprocess.check_output([harness, "R"], text=True)
+    rows = [line.split() for line in out.strip().splitlines()]
+    assert [int(r[1]) for r in rows] == [16, 20, 24, 32, 40, 48, 64, 80, 128, 160, 180, 192, 240, 256, 320]
+    for r in rows:
+        v = list(map(float, r[2:]))
+        for f32 in v[0:2] + v[4:6]:
+            assert f32 < 5e-7, r
+        for f64 in v[2:4] + v[6:8]:
+            assert f64 < 5e-15, r
