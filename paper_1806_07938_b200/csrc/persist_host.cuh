@@ -20,7 +20,7 @@ struct PersistState {
     void *d_xd = nullptr, *d_rd = nullptr, *d_pd = nullptr, *d_bd = nullptr;
     double *d_part_r = nullptr, *d_part_s = nullptr, *d_part_i = nullptr;
     int G = 0, nq_m = 1, NQ = 0, SB = 0, any_remove = 0, spec_smem = 0, vec_smem = 0;
-    int off_ms = 0, off_work = 0, off_red = 0, off_scal = 0, off_tab = 0, off_upart = 0, off_vm = 0, off_vec = 0, off_spec = 0, off_ptab = 0, ngs = 2;
+    int off_ms = 0, off_work = 0, off_red = 0, off_scal = 0, off_tab = 0, off_upart = 0, off_vm = 0, off_vec = 0, off_spec = 0, off_ptab = 0, off_unit = 0, ngs = 2;
     size_t smem = 0;
     bool attr_set = false;
 };
@@ -59,7 +59,7 @@ static int persist_launch(tomo_plan *pl, cudaStream_t st, const PLaunch &L) {
     a.spec_smem = ps->spec_smem; a.vec_smem = ps->vec_smem; a.any_remove = ps->any_remove;
     a.off_ms = ps->off_ms; a.off_work = ps->off_work; a.off_red = ps->off_red; a.off_scal = ps->off_scal;
     a.off_tab = ps->off_tab; a.off_upart = ps->off_upart; a.off_vm = ps->off_vm; a.off_vec = ps->off_vec;
-    a.off_spec = ps->off_spec; a.off_ptab = ps->off_ptab; a.ngs = ps->ngs;
+    a.off_spec = ps->off_spec; a.off_ptab = ps->off_ptab; a.off_unit = ps->off_unit; a.ngs = ps->ngs;
     a.s_in = L.slopes; a.x0 = L.x0;
     a.x = (T *)pl->d_x; a.r = (T *)pl->d_r; a.p = (T *)pl->d_p;
     a.xd = (T *)ps->d_xd; a.rd = (T *)ps->d_rd; a.pd = (T *)ps->d_pd; a.bd = (T *)ps->d_bd;

@@ -61,7 +61,7 @@ template <typename T, typename S> struct PArgs {
     int vec_smem;                // x, r, p rows of the CTA's units held in shared memory for the whole solve
     int any_remove;
     // shared-memory layout (byte offsets)
-    int off_ms, off_work, off_red, off_scal, off_tab, off_upart, off_vm, off_vec, off_spec, off_ptab;
+    int off_ms, off_work, off_red, off_scal, off_tab, off_upart, off_vm, off_vec, off_spec, off_ptab, off_unit;
     int ngs;                     // row-unit buffer slots in shared memory = row units processed per round
     const float *s_in;           // [F][C][nv] slopes (COLD/WARM)
     const float *x0;             // [F][C][nv] warm start (WARM)
@@ -136,21 +136,23 @@ __device__ __forceinline__ double2 shfl_c(double2 v, int src) {
     return make_double2(__shfl_sync(0xffffffffu, v.x, src), __shfl_sync(0xffffffffu, v.y, src));
 }
 
-// ---- the two codelets: R-point DFT from src (stride ss) to dst (stride ds), optional twiddle tw[tj * k]
+// ---- the two codelets: R-point DFT from src (stride ss; only the first nin inputs are read, the rest are zero: the
+// padding of Eq.18-19 is never stored) to dst (stride ds), optional twiddle tw[tj * k]
 template <typename T, int R, bool TW>
-__device__ __noinline__ void dft_pass(const typename cx_of<T>::type *src, int ss, typename cx_of<T>::type *dst, int ds,
+__device__ __noinline__ void dft_pass(const typename cx_of<T>::type *src, int ss, int nin, typename cx_of<T>::type *dst, int ds,
                                       const typename cx_of<T>::type *tw, int tj) {
     typedef typename cx_of<T>::type C2;
     C2 v[R];
 #pragma unroll
-    for (int j = 0; j < R; ++j) v[j] = src[j * ss];
+    for (int j = 0; j < R; ++j) v[j] = (j < nin) ? src[j * ss] : mk<T>((T)0, (T)0);
     SmallDft<T, R, false>::run(v);
     dst[0] = v[0];
 #pragma unroll
     for (int k = 1; k < R; ++k) dst[k * ds] = TW ? cmul(v[k], tw[tj * k]) : v[k];
 }
 
-struct PairRef { int off; float sgn; };          // spectrum block of (c_out, c_in): element offset and conjugation sign
+struct PairRef { int off; float sgn; };
+struct UnitRec { int f, c, j, s0, s1, s2, pad0, pad1; };   // row unit of a CTA: frame, channel, row pair, valid-list range          // spectrum block of (c_out, c_in): element offset and conjugation sign
 
 // ---- per-frequency block product of one k_x slab (Eq.22, Eq.30) + Sigma_eta (L260) + Parseval partials.
 // Warps are grouped: WPG = ceil(P/32) warps cover the k_y range, group g owns a contiguous range of output channels.
@@ -179,22 +181,41 @@ __device__ __forceinline__ void mac_slab(const typename cx_of<T>::type *X, typen
         for (int ci = 0; ci < CT; ++ci) x[ci] = X[ci * LD + ky];
     }
     T pap = (T)0;
-#pragma unroll 1
-    for (int oc = oc_lo; oc < oc_hi; ++oc) {
-        const C2 xo = X[oc * LD + ky];
-        const T s2 = s2c[oc];
-        const PairRef *row = ptab + oc * C;
-        T ar = s2 * xo.x, ai = s2 * xo.y;
-        if (CT > 0) {
+    if constexpr (CT > 0) {
+        // every pair index and conjugation is a compile-time constant; a warp runs only its own range of rows
 #pragma unroll
-            for (int ci = 0; ci < CT; ++ci) {
-                const PairRef e = row[ci];
-                const S2 s = sp[e.off];
-                const T sr = (T)s.x, si = (T)s.y * (T)e.sgn;
-                ar += sr * x[ci].x - si * x[ci].y;
-                ai += sr * x[ci].y + si * x[ci].x;
+        for (int oc = 0; oc < CT; ++oc) {
+            if (oc >= oc_lo && oc < oc_hi) {
+                const T s2 = s2c[oc];
+                T ar = s2 * x[oc].x, ai = s2 * x[oc].y;
+#pragma unroll
+                for (int ci = 0; ci < CT; ++ci) {
+                    const int lo = ci < oc ? ci : oc, hi = ci < oc ? oc : ci;
+                    const S2 s = sp[(lo * CT - (lo * (lo - 1)) / 2 + hi - lo) * P];
+                    const T sr = (T)s.x, si = (T)s.y;
+                    if (ci < oc) {           // conjugate of the stored block
+                        ar += sr * x[ci].x + si * x[ci].y;
+                        ai += sr * x[ci].y - si * x[ci].x;
+                    } else {
+                        ar += sr * x[ci].x - si * x[ci].y;
+                        ai += sr * x[ci].y + si * x[ci].x;
+                    }
+                }
+                Y[oc * LD + ky] = mk<T>(ar, -ai);
+                pap += x[oc].x * ar + x[oc].y * ai;                       // Re(conj(p~) y~)
+                if (any_remove) {
+                    red_s[oc * P + ky] = m0.x * ar + m0.y * ai;           // Re(conj(m~) y~)
+                    if (nq_m > 1) { const C2 mm = (oc & 1) ? m2 : m1; red_f[oc * P + ky] = mm.x * ar + mm.y * ai; }
+                }
             }
-        } else {
+        }
+    } else {
+#pragma unroll 1
+        for (int oc = oc_lo; oc < oc_hi; ++oc) {
+            const C2 xo = X[oc * LD + ky];
+            const T s2 = s2c[oc];
+            const PairRef *row = ptab + oc * C;
+            T ar = s2 * xo.x, ai = s2 * xo.y;
             for (int ci = 0; ci < C; ++ci) {
                 const PairRef e = row[ci];
                 const S2 s = sp[e.off];
@@ -203,12 +224,12 @@ __device__ __forceinline__ void mac_slab(const typename cx_of<T>::type *X, typen
                 ar += sr * xv.x - si * xv.y;
                 ai += sr * xv.y + si * xv.x;
             }
-        }
-        Y[oc * LD + ky] = mk<T>(ar, -ai);
-        pap += xo.x * ar + xo.y * ai;                               // Re(conj(p~) y~)
-        if (any_remove) {
-            red_s[oc * P + ky] = m0.x * ar + m0.y * ai;             // Re(conj(m~) y~)
-            if (nq_m > 1) { const C2 mm = (oc & 1) ? m2 : m1; red_f[oc * P + ky] = mm.x * ar + mm.y * ai; }
+            Y[oc * LD + ky] = mk<T>(ar, -ai);
+            pap += xo.x * ar + xo.y * ai;
+            if (any_remove) {
+                red_s[oc * P + ky] = m0.x * ar + m0.y * ai;
+                if (nq_m > 1) { const C2 mm = (oc & 1) ? m2 : m1; red_f[oc * P + ky] = mm.x * ar + mm.y * ai; }
+            }
         }
     }
     red[grp * P + ky] = pap;
@@ -246,6 +267,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
     T *svec = reinterpret_cast<T *>(smem_raw + a.off_vec);
     S2 *sspec = reinterpret_cast<S2 *>(smem_raw + a.off_spec);
     PairRef *ptab = reinterpret_cast<PairRef *>(smem_raw + a.off_ptab);
+    UnitRec *s_unit = reinterpret_cast<UnitRec *>(smem_raw + a.off_unit);
     C2 *Ubuf = work, *Vbuf = work + (size_t)C * LD;
     const int NGS = a.ngs;
     C2 *bufA = work + (size_t)(gs < NGS ? gs : 0) * (P + LD), *bufB = bufA + P;   // row unit: natural [P], pass-1 result [LD]
@@ -296,8 +318,17 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
     }
     for (int i = tid; i < F * SB; i += kPThreads) scal[i] = 0.0;
     for (int i = tid; i < nu * kGS; i += kPThreads) s_vm[i] = 0u;
+    for (int i = tid; i < (nu > 0 ? nu : 1); i += kPThreads) {
+        UnitRec u;
+        const int ut = min(b + i * G, F * U - 1);
+        u.f = ut / U;
+        const int uu = ut - u.f * U;
+        u.c = uu / npairs; u.j = uu - u.c * npairs;
+        u.s0 = a.g.row_ptr[2 * u.j]; u.s1 = a.g.row_ptr[2 * u.j + 1]; u.s2 = a.g.row_ptr[min(2 * u.j + 2, n)];
+        u.pad0 = u.pad1 = 0;
+        s_unit[i] = u;
+    }
     __syncthreads();
-    const S2 *spec = a.spec_smem ? sspec : gspec;
 
     // per-WFS mode coefficients (Z^T Z)^-1 Z^T q from the channel sums (Eq.36): thread t -> (frame, WFS)
     auto mode_coefs = [&](int t) {
@@ -314,15 +345,13 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
     };
 
     struct Unit { int f, c, j, comp, w, y0, s0, s1, s2; bool two; size_t vbase; };
-    auto unit_of = [&](int i) {
+    auto unit_of = [&](int i) {                      // from the table filled above
+        const UnitRec u = s_unit[i];
         Unit q;
-        const int ut = b + i * G;
-        q.f = ut / U;
-        const int u = ut - q.f * U;
-        q.c = u / npairs; q.j = u - q.c * npairs; q.comp = q.c & 1; q.w = q.c >> 1;
-        q.y0 = 2 * q.j; q.two = q.y0 + 1 < n;
-        q.s0 = a.g.row_ptr[q.y0]; q.s1 = a.g.row_ptr[q.y0 + 1]; q.s2 = a.g.row_ptr[min(q.y0 + 2, n)];
-        q.vbase = ((size_t)q.f * C + q.c) * nv;
+        q.f = u.f; q.c = u.c; q.j = u.j; q.comp = u.c & 1; q.w = u.c >> 1;
+        q.y0 = 2 * u.j; q.two = q.y0 + 1 < n;
+        q.s0 = u.s0; q.s1 = u.s1; q.s2 = u.s2;
+        q.vbase = ((size_t)u.f * C + u.c) * nv;
         return q;
     };
     // dense rows (2 x n) of x, r, p, b of unit i
@@ -333,17 +362,18 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
     };
 
     // one P-point transform bufA -> bufA by the 16 lanes of a row-unit group (all 32 lanes of the warp must call)
-    auto unit_fft = [&](bool act) {
+    // (nfill = number of leading elements of bufA that are stored; the rest count as zero)
+    auto unit_fft = [&](bool act, int nfill) {
         __syncwarp();
-        if (act && gl < B) dft_pass<T, A, true>(bufA + gl, B, bufB + gl, B + 1, tw, gl);
+        if (act && gl < B) dft_pass<T, A, true>(bufA + gl, B, (nfill - gl + B - 1) / B, bufB + gl, B + 1, tw, gl);
         __syncwarp();
-        if (act && gl < A) dft_pass<T, B, false>(bufB + gl * (B + 1), 1, bufA + gl, A, tw, 0);
+        if (act && gl < A) dft_pass<T, B, false>(bufB + gl * (B + 1), 1, B, bufA + gl, A, tw, 0);
         __syncwarp();
     };
     // forward x-FFT of the two rows held in bufA (.x = row y0, .y = row y0+1; zero beyond n), split into the two
     // Hermitian half-spectra -> T1
     auto fwd_unit = [&](const Unit &q, bool act) {
-        unit_fft(act);
+        unit_fft(act, n);
         if (act) {
             C2 *out = a.T1 + (((size_t)q.f * Ph) * C + q.c) * npad + q.y0;
             for (int kk = gl; kk < Ph; kk += kGS) {
@@ -358,7 +388,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
         __syncthreads();
         for (int f = tid; f < F; f += kPThreads) {
             double s = 0.0;
-            for (int i = 0; i < nu; ++i) if ((b + i * G) / U == f) s += upart[i];
+            for (int i = 0; i < nu; ++i) if (s_unit[i].f == f) s += upart[i];
             a.part_r[(size_t)f * G + b] = s;
         }
     };
@@ -411,7 +441,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
         __syncwarp();
         if (act) {
             for (int e = gl; e < 2 * n; e += kGS) { ux[e] = (T)0; ur[e] = (T)0; up[e] = (T)0; if (a.mode == PM_WARM) ub[e] = (T)0; }
-            for (int e = gl; e < P; e += kGS) bufA[e] = mk<T>((T)0, (T)0);
+            for (int e = gl; e < n; e += kGS) bufA[e] = mk<T>((T)0, (T)0);
         }
         __syncwarp();
         if (act) {
@@ -440,6 +470,13 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
     // ================================================================ iterations (k = -1 is the warm-start product A x0)
     const int k_begin = (a.mode == PM_WARM) ? -1 : 0;
     const int n_t1 = C * npairs;                        // complex pairs in one T1 slab
+    int voff[2];                                        // slab buffer offset c LD + y of the row pair e2 = tid + 512 m
+    bool vtwo[2];
+#pragma unroll
+    for (int m = 0; m < 2; ++m) {
+        const int e2 = tid + m * kPThreads, c = e2 / npairs, y = 2 * (e2 - c * npairs);
+        voff[m] = c * LD + y; vtwo[m] = y + 1 < n;
+    }
 #pragma unroll 1
     for (k = k_begin; k < a.n_iter; ++k) {
         const bool pre = k < 0;
@@ -487,8 +524,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
             const T beta = (T)sc[SC_BETA];
             C2 *t1p = a.T1p + ((size_t)f * Ph + kx) * C * npad;
             if (f != f_lo) prefetch_slab(f, !take_new);
-            // zero padding rows n..P-1, then p~rows = r~rows + beta p~rows_old on rows 0..n-1 -> Vbuf[c][y]
-            for (int e = tid; e < C * (P - n); e += kPThreads) { const int c = e / (P - n), y = n + e - c * (P - n); Vbuf[c * LD + y] = mk<T>((T)0, (T)0); }
+            // p~rows = r~rows + beta p~rows_old on rows 0..n-1 -> Vbuf[c][y] (the padding rows n..P-1 are never stored)
 #pragma unroll
             for (int m = 0; m < 2; ++m) {
                 const int e2 = tid + m * kPThreads;
@@ -498,32 +534,33 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                     else if (upd) { v0 = mk<T>(n0[m].x + beta * o0[m].x, n0[m].y + beta * o0[m].y); v1 = mk<T>(n1[m].x + beta * o1[m].x, n1[m].y + beta * o1[m].y); }
                     else { v0 = o0[m]; v1 = o1[m]; }
                     if (take_new || upd) st_pair(t1p + 2 * e2, v0, v1);
-                    const int c = e2 / npairs, y = 2 * (e2 - c * npairs);
-                    Vbuf[c * LD + y] = v0;
-                    if (y + 1 < n) Vbuf[c * LD + y + 1] = v1;
+                    Vbuf[voff[m]] = v0;
+                    if (vtwo[m]) Vbuf[voff[m] + 1] = v1;
                 }
             }
             __syncthreads();
             PSTAMP(PT_BUILD);
             // forward y-FFT: pass 1 Vbuf -> Ubuf, pass 2 Ubuf -> Vbuf (natural k_y)
-            if (it1) dft_pass<T, A, true>(Vbuf + c1 * LD + j2s, B, Ubuf + c1 * LD + j2s, B + 1, tw, j2s);
+            if (it1) dft_pass<T, A, true>(Vbuf + c1 * LD + j2s, B, (n - j2s + B - 1) / B, Ubuf + c1 * LD + j2s, B + 1, tw, j2s);
             __syncthreads();
-            if (it2) dft_pass<T, B, false>(Ubuf + c2s * LD + k1s * (B + 1), 1, Vbuf + c2s * LD + k1s, A, tw, 0);
+            if (it2) dft_pass<T, B, false>(Ubuf + c2s * LD + k1s * (B + 1), 1, B, Vbuf + c2s * LD + k1s, A, tw, 0);
             __syncthreads();
             PSTAMP(PT_FFT);
-            switch (C) {
-                case 4: mac_slab<T, S, 4>(Vbuf, Ubuf, LD, spec, ptab, ms, s_s2c, C, P, a.nq_m, a.any_remove, red, warp, lane); break;
-                case 6: mac_slab<T, S, 6>(Vbuf, Ubuf, LD, spec, ptab, ms, s_s2c, C, P, a.nq_m, a.any_remove, red, warp, lane); break;
-                case 8: mac_slab<T, S, 8>(Vbuf, Ubuf, LD, spec, ptab, ms, s_s2c, C, P, a.nq_m, a.any_remove, red, warp, lane); break;
-                case 12: mac_slab<T, S, 12>(Vbuf, Ubuf, LD, spec, ptab, ms, s_s2c, C, P, a.nq_m, a.any_remove, red, warp, lane); break;
-                case 16: mac_slab<T, S, 16>(Vbuf, Ubuf, LD, spec, ptab, ms, s_s2c, C, P, a.nq_m, a.any_remove, red, warp, lane); break;
-                default: mac_slab<T, S, 0>(Vbuf, Ubuf, LD, spec, ptab, ms, s_s2c, C, P, a.nq_m, a.any_remove, red, warp, lane); break;
-            }
+#define TOMO_MAC(CT_, SP_) mac_slab<T, S, CT_>(Vbuf, Ubuf, LD, SP_, ptab, ms, s_s2c, C, P, a.nq_m, a.any_remove, red, warp, lane)
+#define TOMO_MAC_SWITCH(SP_)                                                               \
+    switch (C) {                                                                           \
+        case 4: TOMO_MAC(4, SP_); break;   case 6: TOMO_MAC(6, SP_); break;                \
+        case 8: TOMO_MAC(8, SP_); break;   case 12: TOMO_MAC(12, SP_); break;              \
+        case 16: TOMO_MAC(16, SP_); break; default: TOMO_MAC(0, SP_); break;               \
+    }
+            if (a.spec_smem) { TOMO_MAC_SWITCH(sspec) } else { TOMO_MAC_SWITCH(gspec) }     // shared vs global loads
+#undef TOMO_MAC_SWITCH
+#undef TOMO_MAC
             __syncthreads();
             PSTAMP(PT_MAC);
             // inverse y-FFT as a forward transform of conj(y~): pass 1 Ubuf -> Vbuf; the warps without pass-1 items
             // reduce the slab partials meanwhile
-            if (it1) dft_pass<T, A, true>(Ubuf + c1 * LD + j2s, B, Vbuf + c1 * LD + j2s, B + 1, tw, j2s);
+            if (it1) dft_pass<T, A, true>(Ubuf + c1 * LD + j2s, B, A, Vbuf + c1 * LD + j2s, B + 1, tw, j2s);
             {
                 const int WPG = (P + 31) >> 5, Goc = min(NW / WPG, C);
                 const int slot = NW - 1 - warp;             // free warps are the top ones
@@ -537,15 +574,18 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                 }
             }
             __syncthreads();
-            if (it2) dft_pass<T, B, false>(Vbuf + c2s * LD + k1s * (B + 1), 1, Ubuf + c2s * LD + k1s, A, tw, 0);
+            if (it2) dft_pass<T, B, false>(Vbuf + c2s * LD + k1s * (B + 1), 1, B, Ubuf + c2s * LD + k1s, A, tw, 0);
             __syncthreads();
             // image rows y < n (conjugate back) -> T2[c][y / 2][kx][y & 1]
             {
                 C2 *dst = a.T2 + (size_t)f * C * npairs * Ph * 2 + (size_t)kx * 2;
-                for (int e = tid; e < n_t1; e += kPThreads) {
-                    const int c = e / npairs, y = 2 * (e - c * npairs);
-                    const C2 u0 = Ubuf[c * LD + y], u1 = (y + 1 < n) ? Ubuf[c * LD + y + 1] : mk<T>((T)0, (T)0);
-                    st_pair(dst + (size_t)e * Ph * 2, mk<T>(u0.x, -u0.y), mk<T>(u1.x, -u1.y));
+#pragma unroll
+                for (int m = 0; m < 2; ++m) {
+                    const int e = tid + m * kPThreads;
+                    if (e < n_t1) {
+                        const C2 u0 = Ubuf[voff[m]], u1 = vtwo[m] ? Ubuf[voff[m] + 1] : mk<T>((T)0, (T)0);
+                        st_pair(dst + (size_t)e * Ph * 2, mk<T>(u0.x, -u0.y), mk<T>(u1.x, -u1.y));
+                    }
                 }
             }
             __syncthreads();
@@ -578,7 +618,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                 }
             }
             if (rnd == 0) PSTAMP(PT_R_LOAD);
-            unit_fft(act);
+            unit_fft(act, P);
             if (rnd == 0) PSTAMP(PT_R_FFT1);
             if (rnd == 0) {
                 // scalars: alpha_k, mode coefficients (reduction items from the top warps down)
@@ -608,40 +648,52 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                 const T alpha = (T)sc[SC_ALPHA], beta = (T)sc[SC_BETA];
                 const bool upd = sc[SC_UPD] != 0.0, step = sc[SC_ALPHA] != 0.0;
                 const T c0 = (T)sc[SC_HEAD + 2 * C + q.w * 3 + q.comp], c2 = (T)sc[SC_HEAD + 2 * C + q.w * 3 + 2];
-                T *ux = dense(i, q, 0), *ur = dense(i, q, 1), *up = dense(i, q, 2);
-                const T *ub = dense(i, q, 3);
                 const unsigned vm = s_vm[i * kGS + gl];
-#pragma unroll 1
-                for (int xp = gl, m = 0; xp < P; xp += kGS, ++m) {
-                    T nr[2] = {(T)0, (T)0};
-                    if (xp < n) {
-                        const C2 z = bufA[xp];
+                const T *ub = dense(i, q, 3);
+                // x, r, p of the unit: shared memory (vec_smem) or the dense global rows; separate code so that the
+                // loads and stores are LDS/STS resp. LDG/STG, not generic
+                auto update_rows = [&](T *ux, T *ur, T *up) {
+                    constexpr int NX = (P / 2 + kGS) / kGS;              // columns per lane, n <= P/2 + 1
 #pragma unroll
-                        for (int row = 0; row < 2; ++row) {
-                            if ((vm >> (row * 16 + m)) & 1u) {
-                                const T coord = ((q.comp ? (T)(q.y0 + row) : (T)xp) - half_n) * dd;
-                                const T qp = (row ? -z.y : z.x) - (c0 + c2 * coord);
-                                const int idx = row * n + xp;
-                                T rv;
-                                if (pre) {                                   // warm start: r = b - M_s q, p = r
-                                    rv = ub[idx] - qp;
-                                    ur[idx] = rv; up[idx] = rv;
-                                } else {
-                                    rv = ur[idx];
-                                    T pv = up[idx];
-                                    if (upd) { pv = rv + beta * pv; up[idx] = pv; }
-                                    if (step) {
-                                        ux[idx] += alpha * pv;
-                                        rv -= alpha * qp;
-                                        ur[idx] = rv;
+                    for (int m = 0; m < NX; ++m) {
+                        const int xp = gl + m * kGS;
+                        if (xp < n) {
+                            const C2 z = bufA[xp];
+                            T nr[2] = {(T)0, (T)0};
+#pragma unroll
+                            for (int row = 0; row < 2; ++row) {
+                                if ((vm >> (row * 16 + m)) & 1u) {
+                                    const T coord = ((q.comp ? (T)(q.y0 + row) : (T)xp) - half_n) * dd;
+                                    const T qp = (row ? -z.y : z.x) - (c0 + c2 * coord);
+                                    const int idx = row * n + xp;
+                                    T rv;
+                                    if (pre) {                                   // warm start: r = b - M_s q, p = r
+                                        rv = ub[idx] - qp;
+                                        ur[idx] = rv; up[idx] = rv;
+                                    } else {
+                                        rv = ur[idx];
+                                        T pv = up[idx];
+                                        if (upd) { pv = rv + beta * pv; up[idx] = pv; }
+                                        if (step) {
+                                            ux[idx] += alpha * pv;
+                                            rv -= alpha * qp;
+                                            ur[idx] = rv;
+                                        }
                                     }
+                                    rr += (double)rv * (double)rv;
+                                    nr[row] = rv;
                                 }
-                                rr += (double)rv * (double)rv;
-                                nr[row] = rv;
                             }
+                            bufA[xp] = mk<T>(nr[0], nr[1]);
                         }
                     }
-                    bufA[xp] = mk<T>(nr[0], nr[1]);
+                };
+                if (a.vec_smem) {
+                    T *base = svec + (size_t)i * 6 * n;
+                    update_rows(base, base + 2 * n, base + 4 * n);
+                } else {
+                    const size_t o = (((size_t)q.f * C + q.c) * npad + q.y0) * n;
+                    update_rows(a.xd + o, a.rd + o, a.pd + o);
                 }
             }
             rr = group_sum(rr);

@@ -101,6 +101,8 @@ static int persist_prepare(tomo_plan *pl) {
     off += (size_t)maxu * kGS * sizeof(unsigned);
     ps->off_ptab = (int)(off = align16(off));
     off += (size_t)m.C * m.C * sizeof(PairRef);
+    ps->off_unit = (int)(off = align16(off));
+    off += (size_t)std::max(maxu, 1) * sizeof(UnitRec);
     off = align16(off);
     const size_t spec_bytes = (size_t)m.n_pair * m.P * 2 * SE, vec_bytes = (size_t)maxu * 6 * m.n * E;
     const char *no_pin = getenv("TOMO_NO_SPEC_SMEM"), *no_vec = getenv("TOMO_NO_VEC_SMEM");

@@ -218,7 +218,17 @@ def test_fp64_instantiation_meets_the_literal_gate_where_the_oracle_is_reproduci
     reproducible = k_rep > n_it and rel(phi_b, phi_a) <= 1e-4
     pl = make_plan(name, precision=prec, solver=solver)
     d_w = torch.empty(pl.wavefront_len, dtype=torch.float32, device="cuda")
-    n_gate = n_it if reproducible else max(min(k_rep, n_it) - 2, 3)
+    n_gate = n_it
+    if not reproducible:
+        # the wavefront is 10-1000x more sensitive than the residual history (C_os amplifies the low-order content):
+        # the reproducibility horizon is where BOTH still agree between the two oracle runs, minus 2
+        n_gate = max(min(k_rep, n_it), 3)
+        while n_gate > 3:
+            xa_k, xb_k = osys.solve_cg(s, n_gate)[0], osys.solve_cg(s * (1.0 + 1e-15 * np.cos(np.arange(s.size))), n_gate)[0]
+            if rel(osys.reconstruct(xb_k, 0), osys.reconstruct(xa_k, 0)) <= 1e-4:
+                break
+            n_gate -= 1
+        n_gate = max(n_gate - 2, 3)
     pl.solve(dev(s), d_w, n_gate)
     torch.cuda.synchronize()
     hg = pl.residuals(1, n_gate)[0]
