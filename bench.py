@@ -33,7 +33,7 @@ def parse():
     ap.add_argument("--config", default="cfg3")
     ap.add_argument("--batch", type=int, default=1)
     ap.add_argument("--n-iter", type=int, default=0, help="CG iterations per solve (0 = the config's count)")
-    ap.add_argument("--solver", default=os.environ.get("TOMO_SOLVER", "multikernel"), choices=["multikernel", "persistent"])
+    ap.add_argument("--solver", default=os.environ.get("TOMO_SOLVER", "persistent"), choices=["multikernel", "persistent"])
     ap.add_argument("--precision", default="f32", choices=["f32", "f32s_f64a", "f64"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -266,6 +266,25 @@ def main():
                 "traffic": None, "peak_source": how, "algorithmic_bytes_per_launch": kbytes[dom],
                 "us_per_launch": {k: v * 1e3 for k, v in kt.items()},
                 "state": "in situ inside the iteration loop (spectra L2-resident after the first iteration)"}
+    f_iter = 2 * C * (n * 2.5 * P * np.log2(P) + Ph * 5 * P * np.log2(P)) + 8 * C * C * P * Ph      # SURVEY 8(d), per frame
+    fp32_peak = 148 * 128 * 2 * 1.965e9                                                             # nominal FMA peak, DESIGN.md 6
+    if args.solver == "persistent":
+        # the dominant kernel is the persistent solver itself: device time of the launch alone (CUDA events on the stream)
+        reps = max(3, min(args.steps, 50))
+        k_ms = plan.time_solver(d_slopes, B, n_iter, reps, stream=stream)
+        k_ms0 = plan.time_solver(d_slopes, B, 0, reps, stream=stream)
+        kb = n_iter * b_iter + B * 4 * Ns * E
+        ach = kb / (k_ms * 1e-3) / 1e9
+        roof = {"kernel": "k_persistent", "bound": "hbm", "achieved": ach, "peak": hbm, "unit": "GB/s", "frac": ach / hbm,
+                # dram__bytes_read.sum + dram__bytes_write.sum of one launch, ncu --set full (profiles/r1_persistent_ncu_details.md)
+                "traffic": 8674048 if (cfg.name.startswith("cfg3") and B == 1 and args.precision == "f32") else None,
+                "peak_source": how, "algorithmic_bytes_per_launch": kb,
+                "ms_per_launch": k_ms, "ms_per_launch_n_iter0": k_ms0,
+                "us_per_iteration_in_kernel": (k_ms - k_ms0) / n_iter * 1e3,
+                "alu": {"flop_per_launch": B * n_iter * f_iter, "achieved_TFLOPs": B * n_iter * f_iter / (k_ms * 1e-3) / 1e12,
+                        "peak_TFLOPs": fp32_peak / 1e12, "frac": B * n_iter * f_iter / (k_ms * 1e-3) / fp32_peak},
+                "state": ("one cooperative launch per solve; spectra pinned in shared memory, exchange buffers L2-resident: "
+                          "latency-bound at batch 1 (two grid barriers per iteration), see DESIGN.md 6")}
     iter_roof = {"b_iter_bytes": b_iter, "us_per_iteration": us_iter, "achieved_GBps": b_iter / (us_iter * 1e-6) / 1e9,
                  "frac_of_hbm_peak": b_iter / (us_iter * 1e-6) / 1e9 / hbm}
 

@@ -145,6 +145,13 @@ int tomo_time_kernels(tomo_plan *plan, int n_frames, int n_iter, float *ms_out, 
  * [9] grid barrier A.  The state of the last solve is overwritten. */
 int tomo_time_phases(tomo_plan *plan, int n_frames, int n_iter, float *us_out, void *cuda_stream);
 
+/* Measurement aid (bench.py "roofline" with the persistent solver): `reps` launches of the persistent kernel alone
+ * (A1-A6: rhs projection + n_iter CG iterations from a cold start on `slopes`, device fp32 [n_frames][C][n_vs]; no
+ * target projection), each bracketed by CUDA events on `cuda_stream`; synchronises the stream and returns the mean
+ * device time of one launch in ms (host fp32 [1]). */
+int tomo_time_solver(tomo_plan *plan, const float *slopes, int n_frames, int n_iter, int reps, float *ms_out,
+                     void *cuda_stream);
+
 /* Sizes fixed at plan creation; any pointer may be NULL. */
 int tomo_get_sizes(const tomo_plan *plan, int *n_vs, int *n_vphi, int *slopes_len, int *wavefront_len,
                    int *pad, int *pad_os, int *n_prime);

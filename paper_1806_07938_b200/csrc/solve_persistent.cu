@@ -255,6 +255,29 @@ int time_phases_persistent(tomo_plan *pl, int F, int n_iter, float *us_out, cuda
     return TOMO_OK;
 }
 
+// Measurement aid (tomo_time_solver): the persistent kernel alone, `reps` cold-start launches bracketed by events.
+int time_solver_persistent(tomo_plan *pl, const float *slopes, int F, int n_iter, int reps, float *ms_out, cudaStream_t st) {
+    int rc;
+    if ((rc = persist_prepare(pl))) return rc;
+    std::vector<cudaEvent_t> ev(2 * (size_t)reps);
+    for (auto &e : ev) PCK(cudaEventCreate(&e));
+    for (int i = 0; i < reps && !rc; ++i) {
+        PersistState *ps = (PersistState *)pl->persist;
+        PCK(cudaMemsetAsync(ps->d_flags, 0, 1024, st));     // (the launch below repeats it; keeps the bracket tight)
+        PCK(cudaEventRecord(ev[2 * i], st));
+        rc = persist_dispatch(pl, st, F, n_iter, PM_COLD, 0, slopes, nullptr, nullptr);
+        PCK(cudaEventRecord(ev[2 * i + 1], st));
+    }
+    cudaError_t e = cudaStreamSynchronize(st);
+    double tot = 0.0;
+    for (int i = 0; i < reps; ++i) { float ms = 0.f; cudaEventElapsedTime(&ms, ev[2 * i], ev[2 * i + 1]); tot += ms; }
+    for (auto &x : ev) cudaEventDestroy(x);
+    if (rc) return rc;
+    if (e != cudaSuccess) { set_error(std::string("time_solver: ") + cudaGetErrorString(e)); return TOMO_ECUDA; }
+    *ms_out = (float)(tot / reps);
+    return TOMO_OK;
+}
+
 void persist_destroy(tomo_plan *pl) {
     delete (PersistState *)pl->persist;
     pl->persist = nullptr;

@@ -595,6 +595,7 @@ namespace tomo {
 int solve_persistent(tomo_plan *pl, const float *slopes, float *out, int F, int n_iter, const float *x0, cudaStream_t st);
 int cg_step_persistent(tomo_plan *pl, float *x, float *r, float *p, double *scal, cudaStream_t st);
 int time_phases_persistent(tomo_plan *pl, int F, int n_iter, float *us_out, cudaStream_t st);
+int time_solver_persistent(tomo_plan *pl, const float *slopes, int F, int n_iter, int reps, float *ms_out, cudaStream_t st);
 
 // A7-A8 from the CG solution held in d_x -> d_out (used by the persistent solver)
 int project_from_x(tomo_plan *pl, cudaStream_t st, int F) { return DISPATCH(pl, project_from_x(pl, st, F)); }
@@ -664,6 +665,17 @@ extern "C" int tomo_time_phases(tomo_plan *pl, int n_frames, int n_iter, float *
     if (rc) return rc;
     if (!us_out || n_frames < 1 || n_frames > pl->F || n_iter < 1 || n_iter >= pl->hist_cap) { set_error("bad arguments"); return TOMO_EINVAL; }
     return time_phases_persistent(pl, n_frames, n_iter, us_out, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int tomo_time_solver(tomo_plan *pl, const float *slopes, int n_frames, int n_iter, int reps, float *ms_out,
+                                void *cuda_stream) {
+    int rc = check_ready(pl);
+    if (rc) return rc;
+    if (!slopes || !ms_out || n_frames < 1 || n_frames > pl->F || n_iter < 0 || n_iter >= pl->hist_cap || reps < 1 || reps > 10000) {
+        set_error("bad arguments");
+        return TOMO_EINVAL;
+    }
+    return time_solver_persistent(pl, slopes, n_frames, n_iter, reps, ms_out, (cudaStream_t)cuda_stream);
 }
 
 extern "C" int tomo_get_sizes(const tomo_plan *pl, int *n_vs, int *n_vphi, int *slopes_len, int *wavefront_len,

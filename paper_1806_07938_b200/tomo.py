@@ -23,7 +23,8 @@ TOMO_SOLVER_MULTIKERNEL, TOMO_SOLVER_PERSISTENT = 0, 1
 
 EXPORTS = (
     "tomo_plan_create", "tomo_plan_upload_kernels", "tomo_solve", "tomo_solve_batch", "tomo_apply_css",
-    "tomo_apply_cos", "tomo_cg_step", "tomo_get_zeta", "tomo_time_kernels", "tomo_time_phases", "tomo_get_sizes", "tomo_get_valid_index", "tomo_get_noise",
+    "tomo_apply_cos", "tomo_cg_step", "tomo_get_zeta", "tomo_time_kernels", "tomo_time_phases", "tomo_time_solver",
+    "tomo_get_sizes", "tomo_get_valid_index", "tomo_get_noise",
     "tomo_get_residuals", "tomo_get_stats", "tomo_plan_destroy", "tomo_last_error",
     "tomo_host_sizes", "tomo_host_css_generators", "tomo_host_cos_generators", "tomo_host_generator_spectrum",
     "tomo_host_structure_function",
@@ -89,6 +90,7 @@ def load(build_if_missing: bool = True):
     lib.tomo_get_zeta.argtypes = [vp, fp, C.c_int, vp]
     lib.tomo_time_kernels.argtypes = [vp, C.c_int, C.c_int, C.POINTER(C.c_float), vp]
     lib.tomo_time_phases.argtypes = [vp, C.c_int, C.c_int, C.POINTER(C.c_float), vp]
+    lib.tomo_time_solver.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_float), vp]
     lib.tomo_get_sizes.argtypes = [vp, ip, ip, ip, ip, ip, ip, ip]
     lib.tomo_get_valid_index.argtypes = [vp, ip, ip]
     lib.tomo_get_noise.argtypes = [vp, dp, dp]
@@ -258,6 +260,11 @@ class TomoPlan:
         return dict(zip(("iteration", "rho_beta", "slab_update", "slab_fft_fwd", "slab_mac", "slab_fft_inv", "barrier_b", "alpha_modes",
                          "rows", "barrier_a"),
                         [float(v) for v in us]))
+
+    def time_solver(self, slopes, n_frames: int, n_iter: int, reps: int, stream=None) -> float:
+        ms = (C.c_float * 1)()
+        _check(self.lib.tomo_time_solver(self._h, _ptr(slopes), n_frames, n_iter, reps, ms, _stream_handle(stream)))
+        return float(ms[0])
 
     # -- getters --
     def valid_index(self):
