@@ -129,3 +129,19 @@ def test_printed_closed_forms():
     # unique-element counts (L150, L177, L193)
     assert (2 * n - 1) ** 2 == 25281
     assert abs(tz.ops_css(74, 6, 5.0) / 4.32e9 - 40.6e6 / 4.32e9) < 1e-3
+
+
+def test_rows_from_positions_pin_the_generator_and_direct_sum_routes():
+    """OracleSystem.css_rows_explicit (rows of W Sigma_ss W^T straight from subaperture positions, what the full-size GPU
+    tests sample) = the dense matrix = the generator / direct-sum route used when the dense matrix does not fit."""
+    import numpy as np
+    from oracle.system import OracleSystem
+    from tomo_inputs.configs import small_lgs_config
+    cfg = small_lgs_config(n=10, n_gs=3, n_layers=3)
+    dense = OracleSystem(cfg, build_cos=False)
+    free = OracleSystem(cfg, dense=False, build_cos=False)
+    rows = [0, 17, dense.nv + 3, 5 * dense.nv - 1]
+    R = free.css_rows_explicit(rows)
+    assert np.allclose(R, dense.Css[rows], rtol=0, atol=1e-12 * np.abs(dense.Css).max())
+    u = np.random.default_rng(0).standard_normal(dense.Ns)
+    assert np.allclose(R @ u, free.css_unprojected(u)[rows], rtol=1e-12, atol=1e-10)
