@@ -357,13 +357,13 @@ template <typename T, typename S> struct Ops {
             k_cos_rows_inv<T><<<grid_for(Fn * m.T * m.Kp * ((m.n_p + 1) / 2), kRowWarps), 32 * kRowWarps, rs, st>>>(r);
             LAUNCH_CHECK();
             const size_t total = (size_t)Fn * m.T * m.nvp;
-            k_cos_gather<T><<<(unsigned)std::min<size_t>((total + 255) / 256, 148 * 8), 256, 0, st>>>(
+            k_cos_gather<T><<<(unsigned)std::min<size_t>((total * 8 + 255) / 256, 148 * 8), 256, 0, st>>>(
                 pl->g, Fn, (const T *)pl->d_G, pl->d_interp_i0, (const T *)pl->d_interp_w,
                 (T *)pl->d_phi + (size_t)f0 * m.T * m.nvp);
             LAUNCH_CHECK();
             pl->launches_last += 5;
         }
-        k_phase_project<T><<<dim3(m.T, F), 256, 0, st>>>(pl->g, (const T *)pl->d_phi, pl->d_out);
+        k_phase_project<T><<<dim3(m.T, F), 1024, 0, st>>>(pl->g, (const T *)pl->d_phi, pl->d_out);
         LAUNCH_CHECK();
         pl->launches_last += 1;
         return TOMO_OK;
@@ -387,7 +387,7 @@ template <typename T, typename S> struct Ops {
             ProjectArgs<T, T> pa;
             pa.g = pl->g; pa.in = (const T *)pl->d_x; pa.out = (T *)pl->d_z; pa.out2 = pa.out3 = pa.zero = nullptr;
             pa.partials_r = nullptr; pa.part_stride = 0;
-            k_project<T, T><<<dim3(pl->m.n_wfs, F), 256, 0, st>>>(pa);
+            k_project<T, T><<<dim3(pl->m.n_wfs, F), 1024, 0, st>>>(pa);
             LAUNCH_CHECK();
             pl->launches_last += 1;
             if ((rc = project_targets(pl, st, F))) return rc;
@@ -405,7 +405,7 @@ template <typename T, typename S> struct Ops {
         ProjectArgs<float, T> pa;
         pa.g = pl->g; pa.in = slopes; pa.out = (T *)pl->d_b; pa.out2 = (T *)pl->d_r; pa.out3 = (T *)pl->d_p;
         pa.zero = (T *)pl->d_x; pa.partials_r = pl->d_partials_r; pa.part_stride = pl->part_stride;
-        k_project<float, T><<<dim3(m.n_wfs, F), 256, 0, st>>>(pa);
+        k_project<float, T><<<dim3(m.n_wfs, F), 1024, 0, st>>>(pa);
         LAUNCH_CHECK();
         pl->launches_last += 1;
         int n_part0 = m.n_wfs;
@@ -540,7 +540,7 @@ template <typename T, typename S> struct Ops {
         ProjectArgs<T, T> pa;
         pa.g = pl->g; pa.in = (const T *)pl->d_x; pa.out = (T *)pl->d_z; pa.out2 = pa.out3 = pa.zero = nullptr;
         pa.partials_r = nullptr; pa.part_stride = 0;
-        k_project<T, T><<<dim3(pl->m.n_wfs, F), 256, 0, st>>>(pa);
+        k_project<T, T><<<dim3(pl->m.n_wfs, F), 1024, 0, st>>>(pa);
         LAUNCH_CHECK();
         pl->launches_last += 1;
         return project_targets(pl, st, F);

@@ -22,10 +22,10 @@ template <typename Tin, typename Tout> struct ProjectArgs {
 };
 
 template <typename Tin, typename Tout>
-__global__ void __launch_bounds__(256) k_project(ProjectArgs<Tin, Tout> a) {
-    __shared__ double wred[8][3];
+__global__ void __launch_bounds__(1024) k_project(ProjectArgs<Tin, Tout> a) {
+    __shared__ double wred[32][3];
     __shared__ double coef[3];
-    __shared__ double wsum[8];
+    __shared__ double wsum[32];
     const int w = blockIdx.x, f = blockIdx.y, nv = a.g.nv, n = a.g.n;
     const size_t base = ((size_t)f * a.g.C + 2 * w) * nv;
     const int nr = a.g.n_remove[w];
@@ -245,28 +245,36 @@ __global__ void __launch_bounds__(128) k_cos_rows_inv(CosRowsArgs<T> a) {
 // phi[f][t][p] = sum_k sum_{4 taps} I'_k[p, tap] g_k[tap]   (Eq.16-17, Eq.32)
 template <typename T>
 __global__ void k_cos_gather(DevGeom g, int F, const T *G, const int *i0, const T *wt, T *phi) {
-    const int np = g.n_p, n1 = g.n + 1;
+    // eight lanes per phase point, lane s takes the layers k = s, s + 8, ...; fixed-order (xor tree) sum
+    const int np = g.n_p, n1 = g.n + 1, sub = threadIdx.x & 7;
     const size_t total = (size_t)F * g.T * g.nvp;
-    for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (size_t)gridDim.x * blockDim.x) {
-        const size_t ft = e / g.nvp;
-        const int p = (int)(e - ft * g.nvp);
-        const int px = g.pix[p], py = g.piy[p];
+    const size_t stride = (size_t)gridDim.x * (blockDim.x >> 3);
+    const size_t rounds = (total + stride - 1) / stride;
+    size_t e = (size_t)blockIdx.x * (blockDim.x >> 3) + (threadIdx.x >> 3);
+    for (size_t it = 0; it < rounds; ++it, e += stride) {
         T acc = (T)0;
-        for (int k = 0; k < g.Kp; ++k) {
-            const int ix0 = i0[k * n1 + px], iy0 = i0[k * n1 + py];
-            const T wx = wt[k * n1 + px], wy = wt[k * n1 + py];
-            const T *gk = G + ((ft * g.Kp + k) * np + iy0) * np + ix0;
-            acc += ((T)1 - wy) * (((T)1 - wx) * gk[0] + wx * gk[1]) + wy * (((T)1 - wx) * gk[np] + wx * gk[np + 1]);
+        if (e < total) {
+            const size_t ft = e / g.nvp;
+            const int p = (int)(e - ft * g.nvp);
+            const int px = g.pix[p], py = g.piy[p];
+            for (int k = sub; k < g.Kp; k += 8) {
+                const int ix0 = i0[k * n1 + px], iy0 = i0[k * n1 + py];
+                const T wx = wt[k * n1 + px], wy = wt[k * n1 + py];
+                const T *gk = G + ((ft * g.Kp + k) * np + iy0) * np + ix0;
+                acc += ((T)1 - wy) * (((T)1 - wx) * gk[0] + wx * gk[1]) + wy * (((T)1 - wx) * gk[np] + wx * gk[np + 1]);
+            }
         }
-        phi[e] = acc;
+#pragma unroll
+        for (int o = 4; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        if (e < total && sub == 0) phi[e] = acc;
     }
 }
 
 // A8: phi_hat = M_phi W_phi phi: remove piston (always) and tip/tilt(/focus) over the valid phase points
 // (Eq.35; Z_phi = [1, x, y, x^2+y^2], reading G14).  One CTA per (target, frame); fp32 out.
 template <typename T>
-__global__ void __launch_bounds__(256) k_phase_project(DevGeom g, const T *phi, float *out) {
-    __shared__ double wred[8][4];
+__global__ void __launch_bounds__(1024) k_phase_project(DevGeom g, const T *phi, float *out) {
+    __shared__ double wred[32][4];
     __shared__ double coef[4];
     const size_t base = ((size_t)blockIdx.y * g.T + blockIdx.x) * g.nvp;
     const int nc = 1 + g.n_remove_phase;
