@@ -43,7 +43,9 @@ extern "C" {
 #define TOMO_F64       2       /* everything fp64 (parity gate P-e); the slope / wavefront ABI stays fp32             */
 
 #define TOMO_SOLVER_MULTIKERNEL 0   /* one kernel per phase, whole solve replayed from a CUDA graph                  */
-#define TOMO_SOLVER_PERSISTENT  1   /* one cooperative persistent kernel per solve, device-side grid barriers        */
+#define TOMO_SOLVER_PERSISTENT  1   /* one cooperative persistent kernel per solve, device-side grid barriers;       */
+                                    /* falls back to the multi-kernel solver where it does not apply (FFT edge not   */
+                                    /* instantiated, non-uniform noise diagonal)                                     */
 
 typedef struct tomo_plan tomo_plan;          /* opaque; owns every device allocation it makes                        */
 

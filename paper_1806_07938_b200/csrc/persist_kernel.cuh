@@ -154,12 +154,56 @@ __device__ __noinline__ void dft_pass(const typename cx_of<T>::type *src, int ss
 struct PairRef { int off; float sgn; };
 struct UnitRec { int f, c, j, s0, s1, s2, pad0, pad1; };   // row unit of a CTA: frame, channel, row pair, valid-list range          // spectrum block of (c_out, c_in): element offset and conjugation sign
 
+// ---- the rows [LO, HI) of the block product for one k_y, straight-line: every pair index and conjugation is a
+// compile-time constant, no branch between the rows (the loads of the next row overlap the FMAs of this one)
+template <typename T, typename S, int CT, int PP, int LO, int HI>
+__device__ __forceinline__ void mac_rows(const typename cx_of<T>::type (&x)[CT], const typename cx_of<S>::type *sp, const T *s2c,
+                                         typename cx_of<T>::type *Y, int LD, int ky, typename cx_of<T>::type m0,
+                                         typename cx_of<T>::type m1, typename cx_of<T>::type m2, T *red_s, T *red_f,
+                                         int any_remove, int nq_m, T &pap) {
+    typedef typename cx_of<T>::type C2;
+    typedef typename cx_of<S>::type S2;
+#pragma unroll
+    for (int oc = LO; oc < HI; ++oc) {
+        const T s2 = s2c[oc];
+        T ar = s2 * x[oc].x, ai = s2 * x[oc].y;
+#pragma unroll
+        for (int ci = 0; ci < CT; ++ci) {
+            const int lo = ci < oc ? ci : oc, hi = ci < oc ? oc : ci;
+            const S2 s = sp[(lo * CT - (lo * (lo - 1)) / 2 + hi - lo) * PP];
+            const T sr = (T)s.x, si = (T)s.y;
+            if (ci < oc) {           // conjugate of the stored block
+                ar += sr * x[ci].x + si * x[ci].y;
+                ai += sr * x[ci].y - si * x[ci].x;
+            } else {
+                ar += sr * x[ci].x - si * x[ci].y;
+                ai += sr * x[ci].y + si * x[ci].x;
+            }
+        }
+        Y[oc * LD + ky] = mk<T>(ar, -ai);
+        pap += x[oc].x * ar + x[oc].y * ai;                       // Re(conj(p~) y~)
+        if (any_remove) {
+            red_s[oc * PP + ky] = m0.x * ar + m0.y * ai;          // Re(conj(m~) y~)
+            if (nq_m > 1) { const C2 mm = (oc & 1) ? m2 : m1; red_f[oc * PP + ky] = mm.x * ar + mm.y * ai; }
+        }
+    }
+}
+template <typename T, typename S, int CT, int PP, int G>
+__device__ __forceinline__ void mac_dispatch(int grp, const typename cx_of<T>::type (&x)[CT], const typename cx_of<S>::type *sp,
+                                             const T *s2c, typename cx_of<T>::type *Y, int LD, int ky, typename cx_of<T>::type m0,
+                                             typename cx_of<T>::type m1, typename cx_of<T>::type m2, T *red_s, T *red_f,
+                                             int any_remove, int nq_m, T &pap) {
+    constexpr int WPG = (PP + 31) / 32, GOC = (kPWarps / WPG) < CT ? (kPWarps / WPG) : CT;
+    if (grp == G) mac_rows<T, S, CT, PP, G * CT / GOC, (G + 1) * CT / GOC>(x, sp, s2c, Y, LD, ky, m0, m1, m2, red_s, red_f, any_remove, nq_m, pap);
+    else if constexpr (G + 1 < GOC) mac_dispatch<T, S, CT, PP, G + 1>(grp, x, sp, s2c, Y, LD, ky, m0, m1, m2, red_s, red_f, any_remove, nq_m, pap);
+}
+
 // ---- per-frequency block product of one k_x slab (Eq.22, Eq.30) + Sigma_eta (L260) + Parseval partials.
 // Warps are grouped: WPG = ceil(P/32) warps cover the k_y range, group g owns a contiguous range of output channels.
 // X: forward y-spectra [c][LD] in natural k_y order; Y: [c][LD], CONJUGATED (the inverse transform is run as a forward
 // one).  CT > 0: the C inputs of this k_y are held in registers; CT = 0: run-time channel count.
 // red: [Goc][P] partial p.q, then [C][P] mask sums, then [C][P] focus sums.
-template <typename T, typename S, int CT>
+template <typename T, typename S, int CT, int PP>
 __device__ __forceinline__ void mac_slab(const typename cx_of<T>::type *X, typename cx_of<T>::type *Y, int LD,
                                          const typename cx_of<S>::type *spec, const PairRef *ptab,
                                          const typename cx_of<T>::type *ms, const T *s2c,
@@ -182,33 +226,7 @@ __device__ __forceinline__ void mac_slab(const typename cx_of<T>::type *X, typen
     }
     T pap = (T)0;
     if constexpr (CT > 0) {
-        // every pair index and conjugation is a compile-time constant; a warp runs only its own range of rows
-#pragma unroll
-        for (int oc = 0; oc < CT; ++oc) {
-            if (oc >= oc_lo && oc < oc_hi) {
-                const T s2 = s2c[oc];
-                T ar = s2 * x[oc].x, ai = s2 * x[oc].y;
-#pragma unroll
-                for (int ci = 0; ci < CT; ++ci) {
-                    const int lo = ci < oc ? ci : oc, hi = ci < oc ? oc : ci;
-                    const S2 s = sp[(lo * CT - (lo * (lo - 1)) / 2 + hi - lo) * P];
-                    const T sr = (T)s.x, si = (T)s.y;
-                    if (ci < oc) {           // conjugate of the stored block
-                        ar += sr * x[ci].x + si * x[ci].y;
-                        ai += sr * x[ci].y - si * x[ci].x;
-                    } else {
-                        ar += sr * x[ci].x - si * x[ci].y;
-                        ai += sr * x[ci].y + si * x[ci].x;
-                    }
-                }
-                Y[oc * LD + ky] = mk<T>(ar, -ai);
-                pap += x[oc].x * ar + x[oc].y * ai;                       // Re(conj(p~) y~)
-                if (any_remove) {
-                    red_s[oc * P + ky] = m0.x * ar + m0.y * ai;           // Re(conj(m~) y~)
-                    if (nq_m > 1) { const C2 mm = (oc & 1) ? m2 : m1; red_f[oc * P + ky] = mm.x * ar + mm.y * ai; }
-                }
-            }
-        }
+        mac_dispatch<T, S, CT, PP, 0>(grp, x, sp, s2c, Y, LD, ky, m0, m1, m2, red_s, red_f, any_remove, nq_m, pap);
     } else {
 #pragma unroll 1
         for (int oc = oc_lo; oc < oc_hi; ++oc) {
@@ -546,7 +564,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
             if (it2) dft_pass<T, B, false>(Ubuf + c2s * LD + k1s * (B + 1), 1, B, Vbuf + c2s * LD + k1s, A, tw, 0);
             __syncthreads();
             PSTAMP(PT_FFT);
-#define TOMO_MAC(CT_, SP_) mac_slab<T, S, CT_>(Vbuf, Ubuf, LD, SP_, ptab, ms, s_s2c, C, P, a.nq_m, a.any_remove, red, warp, lane)
+#define TOMO_MAC(CT_, SP_) mac_slab<T, S, CT_, P>(Vbuf, Ubuf, LD, SP_, ptab, ms, s_s2c, C, P, a.nq_m, a.any_remove, red, warp, lane)
 #define TOMO_MAC_SWITCH(SP_)                                                               \
     switch (C) {                                                                           \
         case 4: TOMO_MAC(4, SP_); break;   case 6: TOMO_MAC(6, SP_); break;                \

@@ -615,7 +615,12 @@ extern "C" int tomo_solve_batch(tomo_plan *pl, const float *slopes, float *wavef
     if (n_iter < 0 || n_iter >= pl->hist_cap) { set_error("n_iter outside [0, 1024]"); return TOMO_EINVAL; }
     if (pl->has_cos && !wavefront_out) { set_error("wavefront_out is NULL"); return TOMO_EINVAL; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    if (pl->opt.solver == TOMO_SOLVER_PERSISTENT) return solve_persistent(pl, slopes, wavefront_out, n_frames, n_iter, x0, st);
+    if (pl->opt.solver == TOMO_SOLVER_PERSISTENT) {
+        // FFT edges the persistent kernel is not instantiated for, non-uniform noise, ...: the multi-kernel solver takes over
+        rc = solve_persistent(pl, slopes, wavefront_out, n_frames, n_iter, x0, st);
+        if (rc != TOMO_EUNSUPPORTED) return rc;
+        pl->opt.solver = TOMO_SOLVER_MULTIKERNEL;
+    }
     return DISPATCH(pl, solve(pl, slopes, wavefront_out, n_frames, n_iter, x0, st));
 }
 
@@ -642,7 +647,11 @@ extern "C" int tomo_cg_step(tomo_plan *pl, float *x, float *r, float *p, double 
     int rc = check_ready(pl);
     if (rc) return rc;
     if (!x || !r || !p || !rho_alpha_beta) { set_error("NULL vector"); return TOMO_EINVAL; }
-    if (pl->opt.solver == TOMO_SOLVER_PERSISTENT) return cg_step_persistent(pl, x, r, p, rho_alpha_beta, (cudaStream_t)cuda_stream);
+    if (pl->opt.solver == TOMO_SOLVER_PERSISTENT) {
+        rc = cg_step_persistent(pl, x, r, p, rho_alpha_beta, (cudaStream_t)cuda_stream);
+        if (rc != TOMO_EUNSUPPORTED) return rc;
+        pl->opt.solver = TOMO_SOLVER_MULTIKERNEL;
+    }
     return DISPATCH(pl, cg_step(pl, x, r, p, rho_alpha_beta, (cudaStream_t)cuda_stream));
 }
 

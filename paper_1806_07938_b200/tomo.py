@@ -199,7 +199,7 @@ class TomoPlan:
 
     def __init__(self, cfg, *, noise_frac: Optional[float] = None, sigma2_wfs: Optional[Sequence[float]] = None,
                  slope_model: int = TOMO_HUDGIN, max_batch: int = 1, precision: int = TOMO_F32,
-                 solver: int = TOMO_SOLVER_MULTIKERNEL, build_cos: bool = True, subap_mask=None,
+                 solver: int = TOMO_SOLVER_PERSISTENT, build_cos: bool = True, subap_mask=None,
                  css_gen: Optional[np.ndarray] = None, cos_gen: Optional[np.ndarray] = None, upload: bool = True):
         self.lib = load()
         self.cfg = cfg

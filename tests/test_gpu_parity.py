@@ -300,3 +300,31 @@ def test_caller_supplied_generators_and_not_ready():
     ref = 2.0 * osys.css_unprojected(v) + osys.sigma2 * v
     assert rel(d_o.cpu().numpy(), ref) <= TOL_MVM
     pl.close()
+
+
+def test_persistent_solver_falls_back_to_the_multikernel_solver_for_other_fft_edges():
+    """n = 25 pads to P = 50 = 2 * 5^2, an edge the persistent kernel is not instantiated for: the default solver must hand
+    over to the multi-kernel path (include/tomo.h) and still meet the gates."""
+    cfg = small_lgs_config(n=25, n_gs=3, n_layers=3, targets=((0.0, 0.0),))
+    osys = OracleSystem(cfg)
+    data = screens.generate(cfg, osys.sigma2, n_frames=1)
+    s = f32(data["slopes"][0].ravel())
+    pl = tomo.TomoPlan(cfg)                     # default: persistent
+    assert pl.P == 50
+    d_w = torch.empty(pl.wavefront_len, dtype=torch.float32, device="cuda")
+    n_it = 8
+    pl.solve(dev(s), d_w, n_it)
+    torch.cuda.synchronize()
+    assert pl.stats()["launches_last_solve"] > 4 * n_it          # one launch per phase, not one per solve
+    x_or, h_or = osys.solve_cg(s, n_it)
+    assert np.abs(pl.residuals(1, n_it)[0] / h_or - 1.0).max() <= TOL_TRAJ
+    d_z = torch.empty(osys.Ns, dtype=torch.float32, device="cuda")
+    pl.get_zeta(d_z)
+    torch.cuda.synchronize()
+    assert rel(d_z.cpu().numpy(), x_or) <= TOL_TRAJ
+    # the wavefront of an unconverged iterate amplifies the low-order content of the zeta deviation (DESIGN.md 4):
+    # the projection is gated on the oracle's iterate
+    pl.apply_cos(dev(x_or), d_w)
+    torch.cuda.synchronize()
+    assert rel(d_w.cpu().numpy(), osys.reconstruct(f32(x_or), 0)) <= TOL_MVM
+    pl.close()
