@@ -646,9 +646,10 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                     if (lane == 0) scal[f * SB + (qq == 0 ? SC_PQ : SC_HEAD + qq - 1)] = s;
                 }
                 __syncthreads();
-                for (int t = tid; t < F * N; t += kPThreads) mode_coefs(t);
-                if (!pre && tid >= 32 * (NW - 1) && tid - 32 * (NW - 1) < F) {       // last warp: alpha per frame
-                    for (int f = tid - 32 * (NW - 1); f < F; f += 32) {
+                // alpha_k is recorded for the next phase C / the tail; every row unit derives alpha and its own mode
+                // coefficients from the sums itself (a few fp64 operations per lane beat a serial section + a barrier)
+                if (!pre) {
+                    for (int f = tid; f < F; f += kPThreads) {
                         double *sc = scal + f * SB;
                         const double rho = sc[SC_RHO], pq = sc[SC_PQ];
                         const double al = (rho > 0.0 && pq > 0.0) ? div_as<T>(rho, pq) : 0.0;     // breakdown: freeze (reading G16)
@@ -656,16 +657,28 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                         if (b == 0) a.alpha[f] = al;
                     }
                 }
-                __syncthreads();
                 PSTAMP(PT_SCAL);
             }
             // stage 2: q' = M_s q, CG vector updates, r.r partial, the new residual rows -> bufA -> forward x-FFT -> T1
             double rr = 0.0;
             if (act) {
                 const double *sc = scal + q.f * SB;
-                const T alpha = (T)sc[SC_ALPHA], beta = (T)sc[SC_BETA];
-                const bool upd = sc[SC_UPD] != 0.0, step = sc[SC_ALPHA] != 0.0;
-                const T c0 = (T)sc[SC_HEAD + 2 * C + q.w * 3 + q.comp], c2 = (T)sc[SC_HEAD + 2 * C + q.w * 3 + 2];
+                const double rho_k = sc[SC_RHO], pq_k = sc[SC_PQ];
+                const double al = (!pre && rho_k > 0.0 && pq_k > 0.0) ? div_as<T>(rho_k, pq_k) : 0.0;   // = sc[SC_ALPHA]
+                const T alpha = (T)al, beta = (T)sc[SC_BETA];
+                const bool upd = sc[SC_UPD] != 0.0, step = al != 0.0;
+                // mode coefficients (Z^T Z)^-1 Z^T q of this unit's WFS from the channel sums (Eq.36)
+                T c0 = (T)0, c2 = (T)0;
+                {
+                    const double *S0 = sc + SC_HEAD, *S1 = sc + SC_HEAD + C;
+                    const double tq[3] = {S0[2 * q.w], S0[2 * q.w + 1], S1[2 * q.w] + S1[2 * q.w + 1]};
+                    const int nr = s_nrem[q.w];
+                    const double *Gw = sGs + q.w * 9;
+                    double d0 = 0.0, d2 = 0.0;
+                    for (int v = 0; v < nr; ++v) { d0 += Gw[q.comp * 3 + v] * tq[v]; d2 += Gw[6 + v] * tq[v]; }
+                    c0 = (q.comp < nr) ? (T)d0 : (T)0;
+                    c2 = (2 < nr) ? (T)d2 : (T)0;
+                }
                 const unsigned vm = s_vm[i * kGS + gl];
                 const T *ub = dense(i, q, 3);
                 // x, r, p of the unit: shared memory (vec_smem) or the dense global rows; separate code so that the
