@@ -74,7 +74,7 @@ template <typename T, typename S> struct PArgs {
     int n_pair;
     const typename cx_of<T>::type *mspec;  // [nq_m][Ph][P]  spectra of the pupil mask (and coordinate-weighted masks)
     const T *s2c;                // [C] sigma^2_c / P^2
-    double *part_r;              // [F][G]       r.r per CTA
+    double *part_r;              // [F][U]       r.r per row unit
     double *part_s;              // [F][NQ][Ph]  per slab: p.q, sum q_c, sum coord q_c
     double *part_i;              // [F][U][2]    init: sum s, sum coord s per row unit
     double *hist;                // [F][hist_stride] rho_k
@@ -114,6 +114,21 @@ __device__ __forceinline__ double warp_sum_cg160(const double *src, int count, i
 #pragma unroll
     for (int m = 0; m < 5; ++m) { const int i = lane + 32 * m; v[m] = (i < count) ? __ldcg(src + i) : 0.0; }
     return warp_sum(((v[0] + v[1]) + (v[2] + v[3])) + v[4]);
+}
+// fixed-order sum by one warp of `count` contiguous doubles other CTAs wrote, 16 loads in flight per lane
+__device__ __forceinline__ double warp_sum_units(const double *src, int count, int lane) {
+    double acc = 0.0;
+    for (int i0 = 0; i0 < count; i0 += 512) {
+        double v[16];
+#pragma unroll
+        for (int m = 0; m < 16; ++m) { const int i = i0 + m * 32 + lane; v[m] = __ldcg(src + min(i, count - 1)); if (i >= count) v[m] = 0.0; }
+#pragma unroll
+        for (int m = 8; m > 0; m >>= 1)
+#pragma unroll
+            for (int j = 0; j < m; ++j) v[j] += v[j + m];
+        acc += v[0];
+    }
+    return warp_sum(acc);
 }
 __device__ __forceinline__ double warp_sum_cg(const double *src, int count, int stride, int lane) {
     double s = 0.0;
@@ -280,7 +295,6 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
     double *sGs = reinterpret_cast<double *>(smem_raw + a.off_tab);
     int *s_nrem = reinterpret_cast<int *>(sGs + 9 * N);
     T *s_s2c = reinterpret_cast<T *>(s_nrem + N + (N & 1));
-    double *upart = reinterpret_cast<double *>(smem_raw + a.off_upart);
     unsigned *s_vm = reinterpret_cast<unsigned *>(smem_raw + a.off_vm);
     T *svec = reinterpret_cast<T *>(smem_raw + a.off_vec);
     S2 *sspec = reinterpret_cast<S2 *>(smem_raw + a.off_spec);
@@ -401,16 +415,6 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
             }
         }
     };
-    // r.r of the CTA's units, per frame, in unit order -> part_r[f][b]
-    auto publish_rr = [&]() {
-        __syncthreads();
-        for (int f = tid; f < F; f += kPThreads) {
-            double s = 0.0;
-            for (int i = 0; i < nu; ++i) if (s_unit[i].f == f) s += upart[i];
-            a.part_r[(size_t)f * G + b] = s;
-        }
-    };
-
     // ================================================================ init (A1: b = M_s s, Eq.33-34)
     // validity bits of the columns x = gl + 16 m each lane updates (bit row * 16 + m) and, for the mode removal, the
     // per-unit sums of s
@@ -479,10 +483,9 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
             }
         }
         rr = group_sum(rr);
-        if (act && gl == 0) upart[i] = rr;
+        if (act && gl == 0) a.part_r[b + i * G] = rr;                   // [f][unit]: unit index b + i G = f U + u
         fwd_unit(q, act);
     }
-    publish_rr();
     GRID_SYNC();
 
     // ================================================================ iterations (k = -1 is the warm-start product A x0)
@@ -520,7 +523,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
             for (int f = NW - 1 - warp; f < F; f += NW) {
                 double rho;
                 if (k == 0 && a.mode == PM_STATE) rho = a.hist[(size_t)f * a.hist_stride];
-                else rho = warp_sum_cg160(a.part_r + (size_t)f * G, G, lane);
+                else rho = warp_sum_units(a.part_r + (size_t)f * U, U, lane);
                 if (lane == 0) {
                     double *sc = scal + f * SB;
                     const double rho_prev = sc[SC_RHO];
@@ -728,12 +731,11 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                 }
             }
             rr = group_sum(rr);
-            if (act && gl == 0) upart[i] = rr;
+            if (act && gl == 0) a.part_r[b + i * G] = rr;                   // [f][unit]: unit index b + i G = f U + u
             if (rnd == 0) PSTAMP(PT_R_UPD);
             fwd_unit(q, act);
             if (rnd == 0) PSTAMP(PT_R_FFT2);
         }
-        publish_rr();
         PSTAMP(PT_ROWS);
         GRID_SYNC();
         PSTAMP(PT_BAR_A);
@@ -744,7 +746,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
     for (int f = NW - 1 - warp; f < F; f += NW) {
         double rho;
         if (a.n_iter == 0 && a.mode == PM_STATE) rho = a.hist[(size_t)f * a.hist_stride];
-        else rho = warp_sum_cg160(a.part_r + (size_t)f * G, G, lane);
+        else rho = warp_sum_units(a.part_r + (size_t)f * U, U, lane);
         if (lane == 0) {
             double *sc = scal + f * SB;
             const double rho_prev = sc[SC_RHO];

@@ -128,7 +128,7 @@ static int persist_prepare(tomo_plan *pl) {
     PTRY(palloc(pl, &ps->d_rd, dsz));
     PTRY(palloc(pl, &ps->d_pd, dsz));
     PTRY(palloc(pl, &ps->d_bd, dsz));
-    PTRY(palloc(pl, (void **)&ps->d_part_r, (size_t)F * sms * sizeof(double)));
+    PTRY(palloc(pl, (void **)&ps->d_part_r, (size_t)F * U * sizeof(double)));
     PTRY(palloc(pl, (void **)&ps->d_part_s, (size_t)F * m.Ph * ps->NQ * sizeof(double)));
     PTRY(palloc(pl, (void **)&ps->d_part_i, (size_t)F * U * 2 * sizeof(double)));
     PTRY(palloc(pl, &ps->d_mspec, (size_t)ps->nq_m * m.Ph * m.P * 2 * E));
