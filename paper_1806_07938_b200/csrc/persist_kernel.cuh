@@ -187,12 +187,13 @@ __device__ __forceinline__ void mac_rows(const typename cx_of<T>::type (&x)[CT],
             const int lo = ci < oc ? ci : oc, hi = ci < oc ? oc : ci;
             const S2 s = sp[(lo * CT - (lo * (lo - 1)) / 2 + hi - lo) * PP];
             const T sr = (T)s.x, si = (T)s.y;
+            // four dependent-free FMAs per complex product ("ar += a*b - c*d" compiles to FMUL + FFMA + FADD)
             if (ci < oc) {           // conjugate of the stored block
-                ar += sr * x[ci].x + si * x[ci].y;
-                ai += sr * x[ci].y - si * x[ci].x;
+                ar = fma(sr, x[ci].x, ar); ar = fma(si, x[ci].y, ar);
+                ai = fma(sr, x[ci].y, ai); ai = fma(-si, x[ci].x, ai);
             } else {
-                ar += sr * x[ci].x - si * x[ci].y;
-                ai += sr * x[ci].y + si * x[ci].x;
+                ar = fma(sr, x[ci].x, ar); ar = fma(-si, x[ci].y, ar);
+                ai = fma(sr, x[ci].y, ai); ai = fma(si, x[ci].x, ai);
             }
         }
         Y[oc * LD + ky] = mk<T>(ar, -ai);
@@ -254,8 +255,8 @@ __device__ __forceinline__ void mac_slab(const typename cx_of<T>::type *X, typen
                 const S2 s = sp[e.off];
                 const C2 xv = X[ci * LD + ky];
                 const T sr = (T)s.x, si = (T)s.y * (T)e.sgn;
-                ar += sr * xv.x - si * xv.y;
-                ai += sr * xv.y + si * xv.x;
+                ar = fma(sr, xv.x, ar); ar = fma(-si, xv.y, ar);
+                ai = fma(sr, xv.y, ai); ai = fma(si, xv.x, ai);
             }
             Y[oc * LD + ky] = mk<T>(ar, -ai);
             pap += xo.x * ar + xo.y * ai;
