@@ -12,7 +12,7 @@ What it computes (each module cites the passage it follows, PAPER.md L<line>):
   covariance.py  linear-stencil slope models (Eq.47-48, Eq.54-55), dense C_ss (Eq.14,
                  L136-158) and C_os (Eq.15-17, L170-197) built from POSITIONS
   projectors.py  W, Z, M = I - Z Z^+ (Eq.33-36)
-  solver.py      direct solve of Eq.5/Eq.12 and textbook CG (S2.G L337), Eq.13
+  solver.py      direct solve of Eq.5/Eq.12, textbook CG and MINRES (S2.G L337, L426), Eq.13
   toeplitz.py    the paper's 2RBT product Eq.18-28 step by step, generators, op counts
   directsum.py   matrix-free direct-sum MVM for ELT sizes (directsum.c, OpenMP)
   system.py      assembles a TomoConfig into the operator A, rhs and projections
@@ -20,7 +20,8 @@ What it computes (each module cites the passage it follows, PAPER.md L<line>):
 Pins (tests/test_oracle_*.py, `-m "not gpu"`): closed forms of D_phi, the Kolmogorov
 limit, the PSD integral, printed formulas Eq.50-52 / Eq.56-62 against the generic
 stencil evaluation, symmetry/PSD of C_ss, dense == paper's index maps == 2-D FFT
-product, projector identities, CG -> Cholesky, LGS ground-layer identity, the
+product, projector identities, CG -> Cholesky, MINRES = the least-squares minimiser over the
+Krylov space (brute force) = scipy's minres, LGS ground-layer identity, the
 paper's printed closed-form counts (L150, L177, L197, L270, L280, L295).
 
 Parity unpinned: absolute WFE in nm (Table 3), the curves of Fig.9-15 and the FFT

@@ -160,6 +160,16 @@ class OracleSystem:
             f = lambda v: A32 @ v          # noqa: E731  fp32 emulation of the same algorithm
         return solver.cg(f, b, n_iter, x0=x0, dtype=dtype, record=record)
 
+    def solve_minres(self, slopes, n_iter, x0=None, record=False, dtype=np.float64):
+        """Fixed-count MINRES on the same system (the paper's solver for the Toeplitz method, L426)."""
+        b = self.rhs(slopes)
+        if dtype == np.float64:
+            f = self.apply_A
+        else:
+            A32 = self.A.astype(dtype)
+            f = lambda v: A32 @ v          # noqa: E731  fp32 emulation of the same algorithm
+        return solver.minres(f, b, n_iter, x0=x0, dtype=dtype, record=record)
+
     # ------------------------------------------------------------------ projection, Eq.13/35
     def reconstruct(self, zeta, target: int = 0):
         """phi_hat = M_phi W_phi Sigma_{phi s} W_s^T M_s^T zeta over the valid phase points."""
