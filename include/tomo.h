@@ -116,6 +116,16 @@ int tomo_solve(tomo_plan *plan, const float *slopes, float *wavefront_out, int n
 int tomo_solve_batch(tomo_plan *plan, const float *slopes, float *wavefront_out, int n_frames, int n_iter,
                      const float *x0, void *cuda_stream);
 
+/* The same path with MINRES instead of CG: the solver the paper keeps for the Toeplitz method (S2.G L337; L426 "MINRES
+ * and CG are used for the Toeplitz and sparse methods"; Fig.13: CG does not converge in its noise-free case).
+ * Paige-Saunders recurrences (Lanczos vectors v_k, Givens rotations of the tridiagonal, directions w_k) around the same
+ * Sigma_ss product kernels, exactly n_iter iterations, no preconditioner, then the projection to every target.
+ * Arguments, layouts, ownership and errors as tomo_solve_batch (x0 = optional warm start, NULL = cold start).
+ * tomo_get_residuals afterwards returns phibar_k = |b - A x_k|, k = 0..n_iter; tomo_get_zeta the iterate x_{n_iter}.
+ * Runs on the multi-kernel solver (one CUDA graph per solve) whatever the plan's `solver` option is. */
+int tomo_solve_minres(tomo_plan *plan, const float *slopes, float *wavefront_out, int n_frames, int n_iter,
+                      const float *x0, void *cuda_stream);
+
 /* out = M_s (W_s Sigma_ss W_s^T + Sigma_eta) M_s^T v  (Eq.30, Eq.34): one product, for the MVM gate.
  * v, out: device fp32 [C][n_vs]. */
 int tomo_apply_css(tomo_plan *plan, const float *v, float *out, void *cuda_stream);

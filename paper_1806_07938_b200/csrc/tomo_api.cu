@@ -10,6 +10,7 @@
 #include "tomo.h"
 #include "tomo_kernels.cuh"
 #include "tomo_kernels_cos.cuh"
+#include "tomo_kernels_minres.cuh"
 #include "tomo_plan.hpp"
 
 namespace tomo {
@@ -455,6 +456,103 @@ template <typename T, typename S> struct Ops {
         return TOMO_OK;
     }
 
+    // ---- MINRES (the paper's solver for the Toeplitz method, S2.G L337, L426): same product kernels, Lanczos + Givens updates
+    static MinresArgs<T> minres_args(tomo_plan *pl, int F, int k, int n_part) {
+        MinresArgs<T> a;
+        a.g = pl->g; a.x = (T *)pl->d_x; a.v = (T *)pl->d_p; a.v_old = (T *)pl->d_vold; a.u = (T *)pl->d_r;
+        a.w1 = (T *)pl->d_w1; a.w2 = (T *)pl->d_w2; a.q = (const T *)pl->d_q; a.partials_q = pl->d_partials_q;
+        a.partials_r = pl->d_partials_r; a.n_part = n_part; a.part_stride = pl->part_stride; a.state = pl->d_mstate;
+        a.alpha = pl->d_alpha; a.hist = pl->d_hist; a.hist_stride = pl->hist_cap; a.k = k; a.F = F;
+        return a;
+    }
+
+    static int enqueue_minres(tomo_plan *pl, cudaStream_t st, int F, int n_iter, int n_part0, bool with_cos) {
+        int rc;
+        const dim3 grid(pl->upd_blocks, F);
+        k_minres_init<T><<<grid, 256, 0, st>>>(minres_args(pl, F, 0, n_part0));
+        LAUNCH_CHECK();
+        pl->launches_last += 1;
+        for (int k = 0; k < n_iter; ++k) {
+            if ((rc = mvm(pl, st, F, 0, 0, 0, 0))) return rc;
+            k_minres_lanczos<T><<<grid, 256, 0, st>>>(minres_args(pl, F, k, pl->upd_blocks));
+            k_minres_update<T><<<grid, 256, 0, st>>>(minres_args(pl, F, k, pl->upd_blocks));
+            LAUNCH_CHECK();
+            pl->launches_last += 2;
+        }
+        if (with_cos) {
+            ProjectArgs<T, T> pa;
+            pa.g = pl->g; pa.in = (const T *)pl->d_x; pa.out = (T *)pl->d_z; pa.out2 = pa.out3 = pa.zero = nullptr;
+            pa.partials_r = nullptr; pa.part_stride = 0;
+            k_project<T, T><<<dim3(pl->m.n_wfs, F), 1024, 0, st>>>(pa);
+            LAUNCH_CHECK();
+            pl->launches_last += 1;
+            if ((rc = project_targets(pl, st, F))) return rc;
+        }
+        return TOMO_OK;
+    }
+
+    static int solve_minres(tomo_plan *pl, const float *slopes, float *out, int F, int n_iter, const float *x0, cudaStream_t st) {
+        const HostModel &m = pl->m;
+        int rc;
+        if ((rc = prepare(pl))) return rc;
+        if (!pl->d_mstate) {
+            const size_t vec = (size_t)pl->F * m.C * m.nv * pl->elem;
+            if ((rc = dev_alloc_bytes(pl, &pl->d_vold, vec))) return rc;
+            if ((rc = dev_alloc_bytes(pl, &pl->d_w1, vec))) return rc;
+            if ((rc = dev_alloc_bytes(pl, &pl->d_w2, vec))) return rc;
+            if ((rc = dev_alloc<double>(pl, &pl->d_mstate, (size_t)2 * pl->F * MS_N))) return rc;
+        }
+        pl->launches_last = 0;
+        const bool with_cos = pl->has_cos && out != nullptr;
+        // A1: b = M_s s -> d_b and d_r (the r0 of a cold start), x = 0, partial b.b  (Eq.33-34)
+        ProjectArgs<float, T> pa;
+        pa.g = pl->g; pa.in = slopes; pa.out = (T *)pl->d_b; pa.out2 = (T *)pl->d_r; pa.out3 = nullptr;
+        pa.zero = (T *)pl->d_x; pa.partials_r = pl->d_partials_r; pa.part_stride = pl->part_stride;
+        k_project<float, T><<<dim3(m.n_wfs, F), 1024, 0, st>>>(pa);
+        LAUNCH_CHECK();
+        pl->launches_last += 1;
+        int n_part0 = m.n_wfs;
+        if (x0) {   // warm start (L428, L506): r0 = b - A x0
+            const size_t cnt = (size_t)F * m.C * m.nv;
+            const unsigned gb = (unsigned)std::min<size_t>((cnt + 255) / 256, 148 * 8);
+            k_convert<float, T><<<gb, 256, 0, st>>>(x0, (T *)pl->d_x, cnt);
+            k_convert<float, T><<<gb, 256, 0, st>>>(x0, (T *)pl->d_p, cnt);
+            LAUNCH_CHECK();
+            if ((rc = mvm(pl, st, F, 0, 0, 0, 0))) return rc;
+            k_warm_residual<T><<<dim3(pl->upd_blocks, F), 256, 0, st>>>(update_args(pl, 0), (const T *)pl->d_b, (T *)pl->d_p);
+            LAUNCH_CHECK();
+            pl->launches_last += 3;
+            n_part0 = pl->upd_blocks;
+        }
+        const auto key = std::make_tuple(F, n_iter, 4 + (x0 ? 1 : 0) + (with_cos ? 2 : 0));
+        auto it = pl->graphs.find(key);
+        const int before = pl->launches_last;
+        if (it == pl->graphs.end()) {
+            cudaStream_t cs;
+            CK(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
+            CK(cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal));
+            rc = enqueue_minres(pl, cs, F, n_iter, n_part0, with_cos);
+            cudaGraph_t graph = nullptr;
+            cudaError_t e = cudaStreamEndCapture(cs, &graph);
+            cudaStreamDestroy(cs);
+            if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+            if (e != cudaSuccess) { set_error(std::string("graph capture: ") + cudaGetErrorString(e)); return TOMO_ECUDA; }
+            cudaGraphExec_t exec = nullptr;
+            e = cudaGraphInstantiate(&exec, graph, 0);
+            cudaGraphDestroy(graph);
+            if (e != cudaSuccess) { set_error(std::string("graph instantiate: ") + cudaGetErrorString(e)); return TOMO_ECUDA; }
+            it = pl->graphs.emplace(key, exec).first;
+            pl->graph_launches[key] = pl->launches_last - before;
+        } else {
+            pl->launches_last += pl->graph_launches[key];
+        }
+        CK(cudaGraphLaunch(it->second, st));
+        if (with_cos)
+            CK(cudaMemcpyAsync(out, pl->d_out, (size_t)F * m.T * m.nvp * sizeof(float), cudaMemcpyDeviceToDevice, st));
+        pl->last_frames = F; pl->last_iter = n_iter;
+        return TOMO_OK;
+    }
+
     static int apply_css(tomo_plan *pl, const float *v, float *out, cudaStream_t st) {
         int rc;
         if ((rc = prepare(pl))) return rc;
@@ -622,6 +720,17 @@ extern "C" int tomo_solve_batch(tomo_plan *pl, const float *slopes, float *wavef
         pl->opt.solver = TOMO_SOLVER_MULTIKERNEL;
     }
     return DISPATCH(pl, solve(pl, slopes, wavefront_out, n_frames, n_iter, x0, st));
+}
+
+extern "C" int tomo_solve_minres(tomo_plan *pl, const float *slopes, float *wavefront_out, int n_frames, int n_iter,
+                                 const float *x0, void *cuda_stream) {
+    int rc = check_ready(pl);
+    if (rc) return rc;
+    if (!slopes) { set_error("slopes is NULL"); return TOMO_EINVAL; }
+    if (n_frames < 1 || n_frames > pl->F) { set_error("n_frames outside [1, max_batch]"); return TOMO_EINVAL; }
+    if (n_iter < 0 || n_iter >= pl->hist_cap) { set_error("n_iter outside [0, 1024]"); return TOMO_EINVAL; }
+    if (pl->has_cos && !wavefront_out) { set_error("wavefront_out is NULL"); return TOMO_EINVAL; }
+    return DISPATCH(pl, solve_minres(pl, slopes, wavefront_out, n_frames, n_iter, x0, (cudaStream_t)cuda_stream));
 }
 
 extern "C" int tomo_solve(tomo_plan *pl, const float *slopes, float *wavefront_out, int n_iter, void *cuda_stream) {

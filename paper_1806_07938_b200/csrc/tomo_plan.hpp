@@ -38,6 +38,9 @@ struct tomo_plan {
     void *d_x = nullptr, *d_r = nullptr, *d_p = nullptr, *d_q = nullptr, *d_b = nullptr;
     void *d_T1 = nullptr, *d_T2 = nullptr;
     double *d_partials_q = nullptr, *d_partials_r = nullptr, *d_hist = nullptr, *d_alpha = nullptr;
+    // MINRES state (allocated by the first tomo_solve_minres): v_{k-1}, w_{k-1}, w_{k-2}, rotation scalars
+    void *d_vold = nullptr, *d_w1 = nullptr, *d_w2 = nullptr;
+    double *d_mstate = nullptr;
     // target projection
     void *d_z = nullptr, *d_T1os = nullptr, *d_Zs = nullptr, *d_T2os = nullptr, *d_G = nullptr, *d_phi = nullptr;
     float *d_out = nullptr;      // [F][T][nvp]

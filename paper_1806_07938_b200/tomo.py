@@ -22,7 +22,7 @@ TOMO_F32, TOMO_F32S_F64A, TOMO_F64 = 0, 1, 2
 TOMO_SOLVER_MULTIKERNEL, TOMO_SOLVER_PERSISTENT = 0, 1
 
 EXPORTS = (
-    "tomo_plan_create", "tomo_plan_upload_kernels", "tomo_solve", "tomo_solve_batch", "tomo_apply_css",
+    "tomo_plan_create", "tomo_plan_upload_kernels", "tomo_solve", "tomo_solve_batch", "tomo_solve_minres", "tomo_apply_css",
     "tomo_apply_cos", "tomo_cg_step", "tomo_get_zeta", "tomo_time_kernels", "tomo_time_phases", "tomo_time_solver",
     "tomo_get_sizes", "tomo_get_valid_index", "tomo_get_noise",
     "tomo_get_residuals", "tomo_get_stats", "tomo_plan_destroy", "tomo_last_error",
@@ -84,6 +84,7 @@ def load(build_if_missing: bool = True):
     lib.tomo_plan_upload_kernels.argtypes = [vp, dp, dp]
     lib.tomo_solve.argtypes = [vp, fp, fp, C.c_int, vp]
     lib.tomo_solve_batch.argtypes = [vp, fp, fp, C.c_int, C.c_int, fp, vp]
+    lib.tomo_solve_minres.argtypes = [vp, fp, fp, C.c_int, C.c_int, fp, vp]
     lib.tomo_apply_css.argtypes = [vp, fp, fp, vp]
     lib.tomo_apply_cos.argtypes = [vp, fp, fp, vp]
     lib.tomo_cg_step.argtypes = [vp, fp, fp, fp, vp, vp]
@@ -236,6 +237,11 @@ class TomoPlan:
         _check(self.lib.tomo_solve_batch(self._h, _ptr(slopes),
                                          _ptr(wavefront_out) if wavefront_out is not None else None, n_frames, n_iter,
                                          None if x0 is None else _ptr(x0), _stream_handle(stream)))
+
+    def solve_minres(self, slopes, wavefront_out, n_frames: int, n_iter: int, x0=None, stream=None):
+        _check(self.lib.tomo_solve_minres(self._h, _ptr(slopes),
+                                          _ptr(wavefront_out) if wavefront_out is not None else None, n_frames, n_iter,
+                                          None if x0 is None else _ptr(x0), _stream_handle(stream)))
 
     def apply_css(self, v, out, stream=None):
         _check(self.lib.tomo_apply_css(self._h, _ptr(v), _ptr(out), _stream_handle(stream)))
