@@ -35,6 +35,8 @@ def parse():
     ap.add_argument("--n-iter", type=int, default=0, help="CG iterations per solve (0 = the config's count)")
     ap.add_argument("--solver", default=os.environ.get("TOMO_SOLVER", "persistent"), choices=["multikernel", "persistent"])
     ap.add_argument("--precision", default="f32", choices=["f32", "f32s_f64a", "f64"])
+    ap.add_argument("--method", default="cg", choices=["cg", "minres"],
+                    help="cg (north_star's solver, the headline) or minres (the paper's solver for the Toeplitz method; multi-kernel path)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
 
@@ -177,6 +179,8 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     prec = {"f32": tomo.TOMO_F32, "f32s_f64a": tomo.TOMO_F32S_F64A, "f64": tomo.TOMO_F64}[args.precision]
+    if args.method == "minres":
+        args.solver = "multikernel"          # tomo_solve_minres runs on the multi-kernel path
     solver = tomo.TOMO_SOLVER_PERSISTENT if args.solver == "persistent" else tomo.TOMO_SOLVER_MULTIKERNEL
     B = args.batch
     t0 = time.perf_counter()
@@ -190,6 +194,13 @@ def main():
     d_out = torch.empty(B * plan.wavefront_len, dtype=torch.float32, device="cuda")
     stream = torch.cuda.current_stream()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
+    minres = args.method == "minres"
+
+    def solve(n_it):
+        if minres:
+            plan.solve_minres(d_slopes, d_out, B, n_it, stream=stream)
+        else:
+            plan.solve_batch(d_slopes, d_out, B, n_it, stream=stream)
 
     def timed(n_it, steps, do_flush=True):
         """device time of `steps` solves, each bracketed by its own CUDA events (the L2 flush is outside)."""
@@ -199,18 +210,18 @@ def main():
                 flush.zero_()
             a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             a.record(stream)
-            plan.solve_batch(d_slopes, d_out, B, n_it, stream=stream)
+            solve(n_it)
             b.record(stream)
             evs.append((a, b))
         torch.cuda.synchronize()
         return sum(a.elapsed_time(b) for a, b in evs)
 
     for _ in range(max(args.warmup, 3)):
-        plan.solve_batch(d_slopes, d_out, B, n_iter, stream=stream)
-        plan.solve_batch(d_slopes, d_out, B, 0, stream=stream)
+        solve(n_iter)
+        solve(0)
     torch.cuda.synchronize()
     launches = plan.stats()["launches_last_solve"]
-    plan.solve_batch(d_slopes, d_out, B, n_iter, stream=stream)
+    solve(n_iter)
     launches = plan.stats()["launches_last_solve"]
 
     sampler = ClockSampler(local_rank)
@@ -229,7 +240,7 @@ def main():
     a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     a.record(stream)
     for _ in range(args.steps):
-        plan.solve_batch(d_slopes, d_out, B, n_iter, stream=stream)
+        solve(n_iter)
     b.record(stream)
     torch.cuda.synchronize()
     ms_step_warm = max_over_ranks(a.elapsed_time(b), world) / args.steps
@@ -239,7 +250,7 @@ def main():
         flush.zero_()
         torch.cuda.synchronize()
         t1 = time.perf_counter()
-        out_h = plan.solve_host(h_slopes, n_iter, n_frames=B, stream=stream)
+        out_h = plan.solve_host(h_slopes, n_iter, n_frames=B, stream=stream, minres=minres)
         stream.synchronize()
         e2e.append(time.perf_counter() - t1)
     e2e_ms = max_over_ranks(statistics.mean(e2e[3:]) * 1e3, world)
@@ -294,7 +305,7 @@ def main():
             "vs_baseline": None, "dtype": args.precision, "data": "synthetic",
             "config": {"workload": cfg.name, "n": cfg.n, "n_wfs": cfg.n_wfs, "n_layers": cfg.n_layers, "pad": plan.P,
                        "pad_os": plan.P_os, "n_iter": n_iter, "batch": B, "targets": len(cfg.targets),
-                       "solver": args.solver, "parallelism": f"replicas x{world}",
+                       "solver": args.solver, "method": args.method, "parallelism": f"replicas x{world}",
                        "l2": "flushed (256 MiB write) before every timed step"},
             "us_per_cg_iteration": us_iter, "ms_per_step_n_iter0": ms_step0, "ms_per_step_l2_warm": ms_step_warm,
             "reconstructions_per_s_l2_warm": world * B * 1e3 / ms_step_warm,

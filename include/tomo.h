@@ -79,6 +79,10 @@ typedef struct {
     double noise_frac;                 /* used when sigma2_wfs == NULL: sigma^2 = noise_frac * model slope variance  */
                                        /* of WFS 0, 1/2 [theta_xx(0) + theta_yy(0)]  (reading G15)                   */
     const double *sigma2_subap;        /* optional host [n_wfs][2][n_vs] full diagonal; overrides both; NULL if unused */
+    const double *sigma_xy_subap;      /* optional host [n_wfs][n_vs]: covariance between the x- and the y-slope noise of   */
+                                       /* one subaperture (elongated LGS spots, L331-333: Sigma_eta becomes 2 x 2 block     */
+                                       /* diagonal); needs sigma2_subap; each block must be positive semi-definite          */
+                                       /* (EINVAL otherwise).  Solved by the multi-kernel solver.  NULL = diagonal noise    */
 } tomo_noise;
 
 typedef struct {

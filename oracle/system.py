@@ -11,7 +11,8 @@ interpolated form sum_k I'_k Xi'_k (Eq.17) for LGS systems.
 Matrix-free mode (ELT sizes, 51 648^2 fp64 = 21 GB dense): the same operator with the
 Sigma_ss product done entry by entry from the generators (directsum.c), no FFT.
 
-Noise (reading G15): Sigma_eta = sigma^2 I, sigma^2 = noise_frac * 1/2 [theta_x0x0(0) + theta_y0y0(0)].
+Noise (reading G15): Sigma_eta = sigma^2 I, sigma^2 = noise_frac * 1/2 [theta_x0x0(0) + theta_y0y0(0)]; optionally the
+2 x 2 block-diagonal Sigma_eta of elongated LGS spots (L331-333), given entry by entry.
 """
 import math
 
@@ -25,7 +26,11 @@ from . import toeplitz as tz
 
 
 class OracleSystem:
-    def __init__(self, cfg, model: str = "hudgin", dense: bool = True, build_cos: bool = True):
+    def __init__(self, cfg, model: str = "hudgin", dense: bool = True, build_cos: bool = True, noise_blocks=None):
+        """noise_blocks = (sxx, syy, sxy), each [n_wfs][n_vs]: Sigma_eta with one 2 x 2 block [[sxx, sxy], [sxy, syy]] per
+        subaperture coupling its x- and y-slope (elongated LGS spots, L331-333); None = sigma^2 I (G15)."""
+        if noise_blocks is not None and not dense:
+            raise ValueError("2 x 2 noise blocks are only assembled in dense mode")
         self.cfg = cfg
         self.model = model
         n, d = cfg.n, cfg.d
@@ -71,7 +76,16 @@ class OracleSystem:
         if dense:
             self.Css = cov.dense_css(self.centres, d, self.dirs, self.hgs, cfg.h, cfg.frac,
                                      cfg.r0, cfg.L0, model)
-            self.A = self.Ms @ (self.Css + self.sigma2 * np.eye(self.Ns)) @ self.Ms.T
+            self.Cnn = self.sigma2 * np.eye(self.Ns)
+            if noise_blocks is not None:
+                sxx, syy, sxy = (np.asarray(a, dtype=np.float64).reshape(self.N, self.nv) for a in noise_blocks)
+                self.Cnn = np.zeros((self.Ns, self.Ns))
+                for i in range(self.N):
+                    for q in range(self.nv):
+                        ex, ey = (2 * i) * self.nv + q, (2 * i + 1) * self.nv + q     # [wfs][x then y][subaperture] (Eq.29)
+                        self.Cnn[ex, ex], self.Cnn[ey, ey] = sxx[i, q], syy[i, q]
+                        self.Cnn[ex, ey] = self.Cnn[ey, ex] = sxy[i, q]
+            self.A = self.Ms @ (self.Css + self.Cnn) @ self.Ms.T
             if build_cos:
                 self.Cos = [self._dense_cos(beta) for beta in cfg.targets]
 

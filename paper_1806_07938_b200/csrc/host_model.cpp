@@ -203,7 +203,17 @@ int build_model(const tomo_geometry *g, const tomo_cn2 *cn2, double r0, double L
             m.sigma2_full[e] = noise->sigma2_subap[e];
         }
         for (int i = 0; i < m.n_wfs; ++i) m.sigma2_wfs[i] = m.sigma2_full[(size_t)2 * i * m.nv];
+        if (noise->sigma_xy_subap) {     // elongated LGS spots (L331-333): 2 x 2 block [[sxx, sxy], [sxy, syy]] per subaperture
+            m.sigma_xy.assign(noise->sigma_xy_subap, noise->sigma_xy_subap + (size_t)m.n_wfs * m.nv);
+            for (int i = 0; i < m.n_wfs; ++i)
+                for (int e = 0; e < m.nv; ++e) {
+                    const double sxx = m.sigma2_full[(size_t)2 * i * m.nv + e], syy = m.sigma2_full[(size_t)(2 * i + 1) * m.nv + e];
+                    const double sxy = m.sigma_xy[(size_t)i * m.nv + e];
+                    if (!(sxy * sxy <= sxx * syy * (1.0 + 1e-12))) { err = "noise block is not positive semi-definite"; return TOMO_EINVAL; }
+                }
+        }
     } else {
+        if (noise && noise->sigma_xy_subap) { err = "sigma_xy_subap needs sigma2_subap"; return TOMO_EINVAL; }
         for (int i = 0; i < m.n_wfs; ++i) {
             double s2 = 0.0;
             if (noise && noise->sigma2_wfs) s2 = noise->sigma2_wfs[i];

@@ -41,6 +41,7 @@ struct HostModel {
     // noise (L110, L260)
     std::vector<double> sigma2_wfs;      // [n_wfs]
     std::vector<double> sigma2_full;     // [C][nv]
+    std::vector<double> sigma_xy;        // [n_wfs][nv] x-y noise covariance per subaperture (L331-333), empty = diagonal noise
     double slope_var = 0;                // 1/2 [theta_x0x0(0) + theta_y0y0(0)]
     // bilinear tables I'_k, separable per axis (Eq.16; reading G18): [Kp][n+1]
     std::vector<int> interp_i0;

@@ -4,6 +4,7 @@
 #include <algorithm>
 #include <cstring>
 #include <string>
+#include <vector>
 
 #include "tomo.h"
 #include "persist_kernel.cuh"
@@ -21,9 +22,16 @@ struct PersistState {
     double *d_part_r = nullptr, *d_part_s = nullptr, *d_part_i = nullptr;
     int G = 0, nq_m = 1, NQ = 0, SB = 0, any_remove = 0, spec_smem = 0, vec_smem = 0;
     int off_ms = 0, off_work = 0, off_red = 0, off_scal = 0, off_tab = 0, off_upart = 0, off_vm = 0, off_vec = 0, off_spec = 0, off_ptab = 0, off_unit = 0, ngs = 2;
+    int off_ms2 = 0;
     size_t smem = 0;
     bool attr_set = false;
+    int *d_seg = nullptr;        // [F_max + 1][sms][8] slab segment tables, one per frame count (slab_segments)
+    std::vector<char> seg_ready; // table for n_frames = f uploaded?
+    int sms = 0;
 };
+
+// balance of the Ph x F slab passes over G CTAs (persist_kernel.cuh, phase C): host table [G][8]
+void slab_segments(int Ph, int F, int G, std::vector<int> &seg);
 
 struct PLaunch {
     int F, n_iter, mode, finalize_p;
@@ -60,6 +68,15 @@ static int persist_launch(tomo_plan *pl, cudaStream_t st, const PLaunch &L) {
     a.off_ms = ps->off_ms; a.off_work = ps->off_work; a.off_red = ps->off_red; a.off_scal = ps->off_scal;
     a.off_tab = ps->off_tab; a.off_upart = ps->off_upart; a.off_vm = ps->off_vm; a.off_vec = ps->off_vec;
     a.off_spec = ps->off_spec; a.off_ptab = ps->off_ptab; a.off_unit = ps->off_unit; a.ngs = ps->ngs;
+    a.off_ms2 = ps->off_ms2;
+    if (!ps->seg_ready[L.F]) {
+        std::vector<int> seg;
+        slab_segments(m.Ph, L.F, a.G, seg);
+        PCK(cudaMemcpyAsync(ps->d_seg + (size_t)L.F * ps->sms * 8, seg.data(), seg.size() * sizeof(int), cudaMemcpyHostToDevice, st));
+        PCK(cudaStreamSynchronize(st));          // the host vector goes out of scope; once per frame count
+        ps->seg_ready[L.F] = 1;
+    }
+    a.seg = ps->d_seg + (size_t)L.F * ps->sms * 8;
     a.s_in = L.slopes; a.x0 = L.x0;
     a.x = (T *)pl->d_x; a.r = (T *)pl->d_r; a.p = (T *)pl->d_p;
     a.xd = (T *)ps->d_xd; a.rd = (T *)ps->d_rd; a.pd = (T *)ps->d_pd; a.bd = (T *)ps->d_bd;

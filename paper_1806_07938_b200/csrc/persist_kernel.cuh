@@ -63,6 +63,8 @@ template <typename T, typename S> struct PArgs {
     // shared-memory layout (byte offsets)
     int off_ms, off_work, off_red, off_scal, off_tab, off_upart, off_vm, off_vec, off_spec, off_ptab, off_unit;
     int ngs;                     // row-unit buffer slots in shared memory = row units processed per round
+    int off_ms2;                 // mask spectra of the helped slab
+    const int *seg;              // [G][8] slab work of a CTA: own frames [0],[1]; helped slab k_x [2], frames [3],[4] (balance)
     const float *s_in;           // [F][C][nv] slopes (COLD/WARM)
     const float *x0;             // [F][C][nv] warm start (WARM)
     T *x, *r, *p;                // [F][C][nv] valid-only layout (ABI side)
@@ -290,6 +292,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
     const int gl = lane & (kGS - 1), gs = tid / kGS;      // lane within the row-unit group, group slot
     C2 *tw = reinterpret_cast<C2 *>(smem_raw);
     C2 *ms = reinterpret_cast<C2 *>(smem_raw + a.off_ms);
+    C2 *ms2 = reinterpret_cast<C2 *>(smem_raw + a.off_ms2);
     C2 *work = reinterpret_cast<C2 *>(smem_raw + a.off_work);
     T *red = reinterpret_cast<T *>(smem_raw + a.off_red);
     double *scal = reinterpret_cast<double *>(smem_raw + a.off_scal);
@@ -311,17 +314,14 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
 #define GRID_SYNC() do { epoch += G; grid_sync(a.flags, epoch); } while (0)
 
     // ---- slab ownership: CTA b owns k_x = b % Ph and a contiguous share of the frames
+    // (the host balances the Ph x F slab passes over the CTAs: a CTA whose own share is below the average also takes
+    // frames of ONE other slab, whose spectra it reads through L2; solve_persistent.cu: slab_segments)
+    // The table row lives in shared memory and is re-read in every phase C, so that it holds no registers across phase R.
     const int kx = b % Ph;
-    int f_lo, f_hi;
-    {
-        const int cnt = (G - 1 - kx) / Ph + 1, rk = b / Ph;
-        f_lo = (int)((long long)rk * F / cnt);
-        f_hi = (int)((long long)(rk + 1) * F / cnt);
-        if (F == 1) { f_lo = 0; f_hi = (rk == 0) ? 1 : 0; }
-    }
-    const bool has_slab = f_hi > f_lo;
-    const S2 *gspec = a.spec + (size_t)kx * a.n_pair * P;
-    const T wkx = (kx == 0 || 2 * kx == P) ? (T)1 : (T)2;
+    volatile int *s_seg = reinterpret_cast<volatile int *>(smem_raw + a.off_ms2 + (size_t)a.nq_m * P * sizeof(C2));
+    if (tid < 8) s_seg[tid] = a.seg[b * 8 + tid];
+    __syncthreads();
+    const bool has_slab = (s_seg[1] - s_seg[0]) + (s_seg[4] - s_seg[3]) > 0;
     // slab thread maps
     const bool it1 = tid < C * B, it2 = tid < C * A;
     const int c1 = tid / B, j2s = tid - c1 * B;      // pass 1: (channel, j2)
@@ -345,9 +345,14 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
     }
     if (has_slab) {
         for (int q = 0; q < a.nq_m; ++q)
-            for (int i = tid; i < P; i += kPThreads) ms[q * P + i] = a.mspec[((size_t)q * Ph + kx) * P + i];
-        if (a.spec_smem)
+            for (int i = tid; i < P; i += kPThreads) {
+                ms[q * P + i] = a.mspec[((size_t)q * Ph + kx) * P + i];
+                ms2[q * P + i] = a.mspec[((size_t)q * Ph + s_seg[2]) * P + i];
+            }
+        if (a.spec_smem && s_seg[1] > s_seg[0]) {
+            const S2 *gspec = a.spec + (size_t)kx * a.n_pair * P;
             for (int i = tid; i < a.n_pair * P; i += kPThreads) sspec[i] = gspec[i];
+        }
     }
     for (int i = tid; i < F * SB; i += kPThreads) scal[i] = 0.0;
     for (int i = tid; i < nu * kGS; i += kPThreads) s_vm[i] = 0u;
@@ -505,10 +510,12 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
         const bool take_new = pre || k == 0;            // p~ = T1 (p_0, or x0 for the warm-start product)
         PSTAMP(PT_START);
         // ---------------------------------------------------------- phase C: slab (kx, f)
+        const int f_lo = s_seg[0], n_own = s_seg[1] - f_lo, kx2 = s_seg[2], f2_lo = s_seg[3], n_items = n_own + s_seg[4] - f2_lo;
         C2 n0[2], n1[2], o0[2], o1[2];
-        auto prefetch_slab = [&](int f, bool with_old) {
-            const C2 *t1 = a.T1 + ((size_t)f * Ph + kx) * C * npad;
-            const C2 *t1p = a.T1p + ((size_t)f * Ph + kx) * C * npad;
+        auto prefetch_slab = [&](int it, bool with_old) {
+            const int f = it < n_own ? f_lo + it : f2_lo + (it - n_own), kxi = it < n_own ? kx : kx2;
+            const C2 *t1 = a.T1 + ((size_t)f * Ph + kxi) * C * npad;
+            const C2 *t1p = a.T1p + ((size_t)f * Ph + kxi) * C * npad;
 #pragma unroll
             for (int m = 0; m < 2; ++m) {
                 const int e2 = tid + m * kPThreads;
@@ -518,7 +525,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                 }
             }
         };
-        if (has_slab) prefetch_slab(f_lo, !take_new);
+        if (has_slab) prefetch_slab(0, !take_new);
         // scalars: rho_k, beta_k (one warp per frame, from the top warp down)
         if (!pre) {
             for (int f = NW - 1 - warp; f < F; f += NW) {
@@ -540,12 +547,16 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
         __syncthreads();
         PSTAMP(PT_RHO);
 #pragma unroll 1
-        for (int f = f_lo; f < f_hi; ++f) {
+        for (int it = 0; it < n_items; ++it) {
+            const bool own = it < n_own;
+            const int f = own ? f_lo + it : f2_lo + (it - n_own), kxi = own ? kx : kx2;
+            const C2 *msi = own ? ms : ms2;
+            const T wkx = (kxi == 0 || 2 * kxi == P) ? (T)1 : (T)2;
             const double *sc = scal + f * SB;
             const bool upd = !pre && sc[SC_UPD] != 0.0;
             const T beta = (T)sc[SC_BETA];
-            C2 *t1p = a.T1p + ((size_t)f * Ph + kx) * C * npad;
-            if (f != f_lo) prefetch_slab(f, !take_new);
+            C2 *t1p = a.T1p + ((size_t)f * Ph + kxi) * C * npad;
+            if (it != 0) prefetch_slab(it, !take_new);
             // p~rows = r~rows + beta p~rows_old on rows 0..n-1 -> Vbuf[c][y] (the padding rows n..P-1 are never stored)
 #pragma unroll
             for (int m = 0; m < 2; ++m) {
@@ -568,14 +579,14 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
             if (it2) dft_pass<T, B, false>(Ubuf + c2s * LD + k1s * (B + 1), 1, B, Vbuf + c2s * LD + k1s, A, tw, 0);
             __syncthreads();
             PSTAMP(PT_FFT);
-#define TOMO_MAC(CT_, SP_) mac_slab<T, S, CT_, P>(Vbuf, Ubuf, LD, SP_, ptab, ms, s_s2c, C, P, a.nq_m, a.any_remove, red, warp, lane)
+#define TOMO_MAC(CT_, SP_) mac_slab<T, S, CT_, P>(Vbuf, Ubuf, LD, SP_, ptab, msi, s_s2c, C, P, a.nq_m, a.any_remove, red, warp, lane)
 #define TOMO_MAC_SWITCH(SP_)                                                               \
     switch (C) {                                                                           \
         case 4: TOMO_MAC(4, SP_); break;   case 6: TOMO_MAC(6, SP_); break;                \
         case 8: TOMO_MAC(8, SP_); break;   case 12: TOMO_MAC(12, SP_); break;              \
         case 16: TOMO_MAC(16, SP_); break; default: TOMO_MAC(0, SP_); break;               \
     }
-            if (a.spec_smem) { TOMO_MAC_SWITCH(sspec) } else { TOMO_MAC_SWITCH(gspec) }     // shared vs global loads
+            if (a.spec_smem && own) { TOMO_MAC_SWITCH(sspec) } else { const S2 *gsp = a.spec + (size_t)kxi * a.n_pair * P; TOMO_MAC_SWITCH(gsp) }     // shared vs global loads
 #undef TOMO_MAC_SWITCH
 #undef TOMO_MAC
             __syncthreads();
@@ -591,7 +602,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                         double s = 0.0;
                         if (tq == 0) s = warp_sum_red<T>(red, Goc * P, lane);
                         else if (a.any_remove) s = warp_sum_red<T>(red + (Goc + tq - 1) * P, P, lane);
-                        if (lane == 0) a.part_s[((size_t)f * NQ + tq) * Ph + kx] = (double)wkx * s;
+                        if (lane == 0) a.part_s[((size_t)f * NQ + tq) * Ph + kxi] = (double)wkx * s;
                     }
                 }
             }
@@ -600,7 +611,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
             __syncthreads();
             // image rows y < n (conjugate back) -> T2[c][y / 2][kx][y & 1]
             {
-                C2 *dst = a.T2 + (size_t)f * C * npairs * Ph * 2 + (size_t)kx * 2;
+                C2 *dst = a.T2 + (size_t)f * C * npairs * Ph * 2 + (size_t)kxi * 2;
 #pragma unroll
                 for (int m = 0; m < 2; ++m) {
                     const int e = tid + m * kPThreads;

@@ -46,6 +46,37 @@ static void build_mask_spectra(const HostModel &m, int nq_m, std::vector<std::co
     }
 }
 
+// Balance of the slab passes of phase C.  CTA b owns slab k_x = b % Ph together with the other CTAs of that residue and
+// takes an even share of the F frames (its spectra stay pinned in shared memory).  With F > 1 the slabs that have one CTA
+// fewer carry up to twice the frames: those CTAs hand the frames beyond the average to CTAs below the average, which
+// process them as a second, "helped" slab with the spectra read through L2.  One helped slab per CTA.
+// seg[b] = {own f_lo, own f_hi, helped k_x, helped f_lo, helped f_hi, 0, 0, 0}.
+void slab_segments(int Ph, int F, int G, std::vector<int> &seg) {
+    seg.assign((size_t)G * 8, 0);
+    std::vector<int> share(G);
+    for (int b = 0; b < G; ++b) {
+        const int kx = b % Ph, cnt = (G - 1 - kx) / Ph + 1, rk = b / Ph;
+        int lo = (int)((long long)rk * F / cnt), hi = (int)((long long)(rk + 1) * F / cnt);
+        if (F == 1) { lo = 0; hi = rk == 0 ? 1 : 0; }
+        seg[b * 8 + 0] = lo; seg[b * 8 + 1] = hi; seg[b * 8 + 2] = kx;
+        share[b] = hi - lo;
+    }
+    const int target = (int)(((long long)Ph * F + G - 1) / G);
+    int h = 0;                                                   // next helper candidate
+    for (int b = 0; b < G; ++b) {
+        while (share[b] > target) {
+            while (h < G && !(share[h] < target && seg[h * 8 + 4] == seg[h * 8 + 3])) ++h;
+            if (h >= G) return;                                  // no helper left: the owner keeps the rest
+            const int take = std::min(share[b] - target, target - share[h]);
+            const int hi = seg[b * 8 + 1];
+            seg[h * 8 + 2] = b % Ph; seg[h * 8 + 3] = hi - take; seg[h * 8 + 4] = hi;
+            seg[b * 8 + 1] = hi - take;
+            share[b] -= take; share[h] += take;
+            ++h;
+        }
+    }
+}
+
 static int persist_prepare(tomo_plan *pl) {
     if (pl->persist) return TOMO_OK;
     const HostModel &m = pl->m;
@@ -56,6 +87,7 @@ static int persist_prepare(tomo_plan *pl) {
                 set_error("persistent solver needs a noise variance that is uniform per WFS channel");
                 return TOMO_EUNSUPPORTED;
             }
+    if (!m.sigma_xy.empty()) { set_error("persistent solver needs a diagonal noise covariance"); return TOMO_EUNSUPPORTED; }
     int dev = 0, sms = 0, coop = 0, max_smem = 0;
     PCK(cudaGetDevice(&dev));
     PCK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
@@ -87,6 +119,8 @@ static int persist_prepare(tomo_plan *pl) {
     size_t off = (size_t)m.P * 2 * E;
     ps->off_ms = (int)(off = align16(off));
     off += (size_t)ps->nq_m * m.P * 2 * E;
+    ps->off_ms2 = (int)(off = align16(off));
+    off += (size_t)ps->nq_m * m.P * 2 * E + 32;      // + the CTA's row of the slab segment table
     ps->off_work = (int)(off = align16(off));
     off += std::max((size_t)2 * m.C * LD, (size_t)ps->ngs * (m.P + LD)) * 2 * E;
     ps->off_red = (int)(off = align16(off));
@@ -121,6 +155,9 @@ static int persist_prepare(tomo_plan *pl) {
     const size_t tsz = (size_t)F * m.Ph * m.C * 2 * npairs * 2 * E;
     const size_t dsz = (size_t)F * m.C * 2 * npairs * m.n * E;
     PTRY(palloc(pl, (void **)&ps->d_flags, 1024));
+    ps->sms = sms;
+    ps->seg_ready.assign((size_t)F + 1, 0);
+    PTRY(palloc(pl, (void **)&ps->d_seg, (size_t)(F + 1) * sms * 8 * sizeof(int)));
     PTRY(palloc(pl, &ps->d_T1, tsz));
     PTRY(palloc(pl, &ps->d_T1p, tsz));
     PTRY(palloc(pl, &ps->d_T2, tsz));

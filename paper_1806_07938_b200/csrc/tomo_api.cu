@@ -130,6 +130,7 @@ extern "C" int tomo_plan_create(const tomo_geometry *geom, const tomo_cn2 *cn2, 
     TRY(upload<double>(pl, &pl->d_Gs, m.Gs));
     TRY(upload<double>(pl, &pl->d_Gphi, m.Gphi));
     TRY(upload_real(pl, &pl->d_sigma2, m.sigma2_full));
+    if (!m.sigma_xy.empty()) TRY(upload_real(pl, &pl->d_sigma_xy, m.sigma_xy));
     TRY(upload_real(pl, &pl->d_interp_w, m.interp_w));
     TRY(upload_twiddles(pl, &pl->d_tw, m.P));
     TRY(upload_twiddles(pl, &pl->d_tw_os, m.P_os));
@@ -315,7 +316,7 @@ template <typename T, typename S> struct Ops {
         prof_mark(pl, st);
         RowsInvArgs<T> b;
         b.st = a.st; b.g = pl->g; b.F = F; b.T2 = (const C2 *)pl->d_T2; b.p = (const T *)pl->d_p;
-        b.sigma2 = (const T *)pl->d_sigma2; b.q = (T *)pl->d_q; b.partials_q = pl->d_partials_q;
+        b.sigma2 = (const T *)pl->d_sigma2; b.sigma_xy = (const T *)pl->d_sigma_xy; b.q = (T *)pl->d_q; b.partials_q = pl->d_partials_q;
         k_rows_inv<T><<<grid_for(items, kRowWarps), 32 * kRowWarps, rows_smem<T>(m.P), st>>>(b);
         LAUNCH_CHECK();
         prof_mark(pl, st);

@@ -6,7 +6,7 @@
 //   cols     : for one kx and ALL channels: length-P FFT along y, per-frequency C x C block product with the
 //              Hermitian-packed kernel spectra (Eq.22, Eq.30), inverse FFT along y -> T2[f][c][kx][y<n]
 //   rows_inv : merge two half-spectra, inverse FFT along x, crop + pupil mask (S_2, W_s; Eq.24-27, Eq.34),
-//              add Sigma_eta p (L260), reduction partials for the mode removal (Eq.36) and p.q
+//              add Sigma_eta p (L260; 2 x 2 blocks for elongated LGS spots, L331-333), reduction partials for the mode removal (Eq.36) and p.q
 //   update   : alpha, x += alpha p, r -= alpha M_s q, partial r.r        (S2.G L337)
 // The next rows_fwd finishes the iteration (beta, p = r + beta p) before scattering p.
 // One warp owns one 1-D transform (fft_device.cuh); kernels are templated on the arithmetic type T and the
@@ -194,6 +194,7 @@ template <typename T> struct RowsInvArgs {
     const typename cx_of<T>::type *T2;   // [F][C][Ph][n]
     const T *p;                          // [F][C][nv]
     const T *sigma2;                     // [C][nv]  diagonal of Sigma_eta
+    const T *sigma_xy;                   // [N][nv]  x-y noise covariance per subaperture (elongated LGS spots, L331-333) or NULL
     T *q;                                // [F][C][nv]  W (Sigma_ss + Sigma_eta) W^T p, modes not yet removed
     double *partials_q;                  // [F][C][npairs][TOMO_NRED]
 };
@@ -231,7 +232,9 @@ __global__ void __launch_bounds__(128) k_rows_inv(RowsInvArgs<T> a) {
             for (int i = s0 + lane; i < e0; i += 32) {
                 const int x = a.g.ix[i];
                 const T pv = a.p[base + i];
-                const T qv = (row ? Z[x].y : Z[x].x) + a.sigma2[(size_t)c * nv + i] * pv;
+                T qv = (row ? Z[x].y : Z[x].x) + a.sigma2[(size_t)c * nv + i] * pv;
+                if (a.sigma_xy)          // 2 x 2 noise block: the other slope component of the same subaperture
+                    qv += a.sigma_xy[(size_t)(c >> 1) * nv + i] * a.p[((size_t)f * C + (c ^ 1)) * nv + i];
                 a.q[base + i] = qv;
                 const T coord = ((comp ? (T)y : (T)x) - half_n) * (T)a.g.d;
                 s_pq += (double)pv * (double)qv; s_q += (double)qv; s_p += (double)pv;

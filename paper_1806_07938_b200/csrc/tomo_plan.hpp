@@ -32,7 +32,7 @@ struct tomo_plan {
     int *d_row_ptr = nullptr, *d_ix = nullptr, *d_iy = nullptr, *d_pix = nullptr, *d_piy = nullptr,
         *d_n_remove = nullptr, *d_interp_i0 = nullptr;
     double *d_Gs = nullptr, *d_Gphi = nullptr;
-    void *d_tw = nullptr, *d_tw_os = nullptr, *d_sigma2 = nullptr, *d_interp_w = nullptr;
+    void *d_tw = nullptr, *d_tw_os = nullptr, *d_sigma2 = nullptr, *d_sigma_xy = nullptr, *d_interp_w = nullptr;
     void *d_spec = nullptr, *d_spec_os = nullptr;
     // CG state and workspaces (arithmetic type T)
     void *d_x = nullptr, *d_r = nullptr, *d_p = nullptr, *d_q = nullptr, *d_b = nullptr;

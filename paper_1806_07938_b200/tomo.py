@@ -54,7 +54,7 @@ class _Cn2(C.Structure):
 
 class _Noise(C.Structure):
     _fields_ = [("sigma2_wfs", C.POINTER(C.c_double)), ("noise_frac", C.c_double),
-                ("sigma2_subap", C.POINTER(C.c_double))]
+                ("sigma2_subap", C.POINTER(C.c_double)), ("sigma_xy_subap", C.POINTER(C.c_double))]
 
 
 class _Options(C.Structure):
@@ -199,17 +199,21 @@ class TomoPlan:
     """tomo_plan_create + tomo_plan_upload_kernels; methods mirror the C entry points one to one."""
 
     def __init__(self, cfg, *, noise_frac: Optional[float] = None, sigma2_wfs: Optional[Sequence[float]] = None,
-                 slope_model: int = TOMO_HUDGIN, max_batch: int = 1, precision: int = TOMO_F32,
+                 sigma2_subap=None, sigma_xy_subap=None, slope_model: int = TOMO_HUDGIN, max_batch: int = 1, precision: int = TOMO_F32,
                  solver: int = TOMO_SOLVER_PERSISTENT, build_cos: bool = True, subap_mask=None,
                  css_gen: Optional[np.ndarray] = None, cos_gen: Optional[np.ndarray] = None, upload: bool = True):
         self.lib = load()
         self.cfg = cfg
         self._pr = _Problem(cfg, subap_mask)
-        if sigma2_wfs is not None:
+        if sigma2_subap is not None:
+            self._s2 = np.ascontiguousarray(sigma2_subap, dtype=np.float64)
+            self._sxy = None if sigma_xy_subap is None else np.ascontiguousarray(sigma_xy_subap, dtype=np.float64)
+            noise = _Noise(None, 0.0, _dp(self._s2), None if self._sxy is None else _dp(self._sxy))
+        elif sigma2_wfs is not None:
             self._s2 = np.ascontiguousarray(sigma2_wfs, dtype=np.float64)
-            noise = _Noise(_dp(self._s2), 0.0, None)
+            noise = _Noise(_dp(self._s2), 0.0, None, None)
         else:
-            noise = _Noise(None, cfg.noise_frac if noise_frac is None else noise_frac, None)
+            noise = _Noise(None, cfg.noise_frac if noise_frac is None else noise_frac, None, None)
         opt = _Options(slope_model, cfg.pad, cfg.pad_os, max_batch, precision, solver, 1 if build_cos else 0)
         self._h = C.c_void_p()
         _check(self.lib.tomo_plan_create(self._pr.geom, self._pr.cn2, cfg.r0, cfg.L0, noise, opt, C.byref(self._h)))
@@ -298,7 +302,7 @@ class TomoPlan:
         return dict(device_bytes=b.value, launches_last_solve=n.value)
 
     # -- convenience: host buffers in, host buffers out (H2D + solve + D2H on one stream) --
-    def solve_host(self, slopes_host, n_iter: int, n_frames: int = 1, stream=None):
+    def solve_host(self, slopes_host, n_iter: int, n_frames: int = 1, stream=None, minres: bool = False):
         """slopes_host: pinned or pageable torch CPU tensor / numpy array [n_frames][C][n_vs] fp32.
         Returns a pinned CPU tensor [n_frames][n_targets][n_vphi]; the caller synchronises the stream."""
         import torch
@@ -314,7 +318,7 @@ class TomoPlan:
         s = stream if stream is not None else torch.cuda.current_stream()
         with torch.cuda.stream(s):
             d_in.copy_(src.reshape(-1), non_blocking=True)
-            self.solve_batch(d_in, d_out, n_frames, n_iter, stream=s)
+            (self.solve_minres if minres else self.solve_batch)(d_in, d_out, n_frames, n_iter, stream=s)
             h_out.copy_(d_out, non_blocking=True)
         return h_out.view(n_frames, self.n_targets, self.n_vphi)
 

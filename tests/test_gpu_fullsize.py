@@ -120,3 +120,34 @@ def test_cfg3_solve_and_projection_against_the_matrix_free_oracle():
     torch.cuda.synchronize()
     assert rel(d_w.cpu().numpy(), osys.reconstruct(f32(x_or), 0)) <= 1e-4
     pl.close()
+
+
+def test_cfg3_batch_with_helped_slabs_equals_single_solves_bitwise():
+    """Batch path at ELT size: with 3 and 5 frames the k_x slabs that have a single CTA hand frames to CTAs of other slabs,
+    which read the spectra through L2 instead of shared memory (persist_kernel.cuh, slab_segments).  Same arithmetic in the
+    same order, so every frame must equal its single-frame solve bit for bit (zeta, residual history, wavefront)."""
+    cfg = get_config("cfg3")
+    B, n_it = 5, 6
+    pl = tomo.TomoPlan(cfg, solver=tomo.TOMO_SOLVER_PERSISTENT, max_batch=B)
+    data = screens.generate(cfg, float(pl.noise()[0][0]), n_frames=B)
+    s = np.ascontiguousarray(data["slopes"].reshape(B, -1), dtype=np.float32)
+    singles = []
+    for f in range(B):
+        d_w = torch.empty(pl.wavefront_len, dtype=torch.float32, device="cuda")
+        d_z = torch.empty(pl.slopes_len, dtype=torch.float32, device="cuda")
+        pl.solve(dev(s[f]), d_w, n_it)
+        pl.get_zeta(d_z)
+        torch.cuda.synchronize()
+        singles.append((d_w.clone(), d_z.clone(), pl.residuals(1, n_it)[0].copy()))
+    for nb in (3, B):
+        d_w = torch.empty(nb * pl.wavefront_len, dtype=torch.float32, device="cuda")
+        d_z = torch.empty(nb * pl.slopes_len, dtype=torch.float32, device="cuda")
+        pl.solve_batch(dev(s[:nb]), d_w, nb, n_it)
+        pl.get_zeta(d_z, nb)
+        torch.cuda.synchronize()
+        h = pl.residuals(nb, n_it)
+        for f in range(nb):
+            assert torch.equal(d_w[f * pl.wavefront_len:(f + 1) * pl.wavefront_len], singles[f][0]), (nb, f)
+            assert torch.equal(d_z[f * pl.slopes_len:(f + 1) * pl.slopes_len], singles[f][1]), (nb, f)
+            assert np.array_equal(h[f], singles[f][2]), (nb, f)
+    pl.close()

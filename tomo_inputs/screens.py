@@ -112,6 +112,44 @@ def generate(cfg: TomoConfig, sigma2: float, n_frames: int = 1, seed_offset: int
                 sub_idx=sidx, phase_idx=pidx, centres=centres, phase_pts=ppts)
 
 
+def elongated_noise_blocks(cfg: TomoConfig, sigma2: float, elongation: float = 2.0):
+    """Synthetic 2 x 2 noise blocks for elongated LGS spots (PAPER.md L331-333 states the structure -- noise that depends on
+    the subaperture position relative to the laser launch telescope, plus an x-y cross term -- but no formula).  Recipe: side
+    launch from the pupil edge towards guide star i, launch_i = D/2 (cos t_i, sin t_i); a subaperture at r sees the spot
+    stretched along e = r - launch_i:  block = sigma2 [I + elongation (|e|/D)^2 e^ e^T].
+    Returns (sxx, syy, sxy), each [n_wfs][n_vs], and `with_noise(slopes_noiseless, frame)` drawing noise of that covariance."""
+    n, d = cfg.n, cfg.d
+    sidx = np.flatnonzero(subap_mask(n, cfg.obstruction).ravel())
+    c1 = (np.arange(n) - (n - 1) / 2.0) * d
+    cx, cy = np.meshgrid(c1, c1, indexing="xy")
+    centres = np.stack([cx.ravel(), cy.ravel()], axis=1)[sidx]
+    sxx, syy, sxy = (np.zeros((cfg.n_wfs, sidx.size)) for _ in range(3))
+    for i, w in enumerate(cfg.wfs):
+        t = math.atan2(w.ay, w.ax)
+        e = centres - 0.5 * cfg.D * np.array([math.cos(t), math.sin(t)])
+        ln = np.maximum(np.hypot(e[:, 0], e[:, 1]), 1e-12)
+        ux, uy = e[:, 0] / ln, e[:, 1] / ln
+        extra = sigma2 * elongation * (ln / cfg.D) ** 2
+        sxx[i], syy[i], sxy[i] = sigma2 + extra * ux * ux, sigma2 + extra * uy * uy, extra * ux * uy
+    return sxx, syy, sxy
+
+
+def add_block_noise(cfg: TomoConfig, slopes_noiseless: np.ndarray, blocks, seed_offset: int = 0) -> np.ndarray:
+    """slopes_noiseless[n_frames, N, 2, n_vs] + zero-mean Gaussian noise with the 2 x 2 covariance blocks (Cholesky factor
+    of each block applied to two i.i.d. normals)."""
+    sxx, syy, sxy = blocks
+    out = np.array(slopes_noiseless, dtype=np.float64, copy=True)
+    l11 = np.sqrt(sxx)
+    l21 = sxy / l11
+    l22 = np.sqrt(np.maximum(syy - l21 * l21, 0.0))
+    for f in range(out.shape[0]):
+        rng = np.random.default_rng(BASE_SEED + 1000 * cfg.cfg_id + 700 + seed_offset + f)
+        z = rng.standard_normal((2,) + sxx.shape)
+        out[f, :, 0] += l11 * z[0]
+        out[f, :, 1] += l21 * z[0] + l22 * z[1]
+    return out
+
+
 def random_vector(cfg: TomoConfig, length: int, seed_offset: int = 0) -> np.ndarray:
     """A seeded white Gaussian vector (for MVM parity on non-slope-like inputs)."""
     rng = np.random.default_rng(BASE_SEED + 1000 * cfg.cfg_id + 900 + seed_offset)
