@@ -24,7 +24,7 @@ struct PersistState {
     int off_ms = 0, off_work = 0, off_red = 0, off_scal = 0, off_tab = 0, off_upart = 0, off_vm = 0, off_vec = 0, off_spec = 0, off_ptab = 0, off_unit = 0, ngs = 2;
     int off_ms2 = 0;
     size_t smem = 0;
-    bool attr_set = false;
+    bool attr_set = false, attr_set_batch = false;
     int *d_seg = nullptr;        // [F_max + 1][sms][8] slab segment tables, one per frame count (slab_segments)
     std::vector<char> seg_ready; // table for n_frames = f uploaded?
     int sms = 0;
@@ -86,16 +86,18 @@ static int persist_launch(tomo_plan *pl, cudaStream_t st, const PLaunch &L) {
     a.part_r = ps->d_part_r; a.part_s = ps->d_part_s; a.part_i = ps->d_part_i;
     a.hist = pl->d_hist; a.hist_stride = pl->hist_cap; a.alpha = pl->d_alpha; a.scal_out = L.scal_out;
     a.flags = ps->d_flags; a.dbg = L.dbg;
-    if (!ps->attr_set) {
-        PCK(cudaFuncSetAttribute((k_persistent<T, S, P>), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ps->smem));
+    const void *kern = L.F > 1 ? (const void *)(k_persistent<T, S, P, true>) : (const void *)(k_persistent<T, S, P, false>);
+    bool &attr_set = L.F > 1 ? ps->attr_set_batch : ps->attr_set;
+    if (!attr_set) {
+        PCK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ps->smem));
         int occ = 0;
-        PCK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (k_persistent<T, S, P>), kPThreads, ps->smem));
+        PCK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kPThreads, ps->smem));
         if (occ < 1) { set_error("persistent kernel does not fit on an SM"); return TOMO_EUNSUPPORTED; }
-        ps->attr_set = true;
+        attr_set = true;
     }
     PCK(cudaMemsetAsync(ps->d_flags, 0, 1024, st));
     void *kargs[] = {&a};
-    PCK(cudaLaunchCooperativeKernel((const void *)(k_persistent<T, S, P>), dim3(a.G), dim3(kPThreads), kargs, ps->smem, st));
+    PCK(cudaLaunchCooperativeKernel(kern, dim3(a.G), dim3(kPThreads), kargs, ps->smem, st));
     pl->launches_last += 1;
     return TOMO_OK;
 }

@@ -278,7 +278,9 @@ template <typename T> __device__ __forceinline__ double warp_sum_red(const T *sr
     return warp_sum((double)s);
 }
 
-template <typename T, typename S, int P>
+// BATCH = false: the single-frame instance (latency-bound: compact code, the CTA's own slab only);
+// BATCH = true: several frames per solve (throughput: balanced slab passes, every global load of a step issued up front)
+template <typename T, typename S, int P, bool BATCH>
 __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
     typedef typename cx_of<T>::type C2;
     typedef typename cx_of<S>::type S2;
@@ -319,7 +321,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
     // The table row lives in shared memory and is re-read in every phase C, so that it holds no registers across phase R.
     const int kx = b % Ph;
     volatile int *s_seg = reinterpret_cast<volatile int *>(smem_raw + a.off_ms2 + (size_t)a.nq_m * P * sizeof(C2));
-    if (tid < 8) s_seg[tid] = a.seg[b * 8 + tid];
+    if (tid < 8) s_seg[tid] = BATCH ? a.seg[b * 8 + tid] : (tid == 1 ? (b < Ph ? 1 : 0) : tid == 2 ? kx : 0);
     __syncthreads();
     const bool has_slab = (s_seg[1] - s_seg[0]) + (s_seg[4] - s_seg[3]) > 0;
     // slab thread maps
@@ -510,7 +512,8 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
         const bool take_new = pre || k == 0;            // p~ = T1 (p_0, or x0 for the warm-start product)
         PSTAMP(PT_START);
         // ---------------------------------------------------------- phase C: slab (kx, f)
-        const int f_lo = s_seg[0], n_own = s_seg[1] - f_lo, kx2 = s_seg[2], f2_lo = s_seg[3], n_items = n_own + s_seg[4] - f2_lo;
+        const int f_lo = BATCH ? s_seg[0] : 0, n_own = BATCH ? s_seg[1] - f_lo : (b < Ph ? 1 : 0), kx2 = BATCH ? s_seg[2] : kx;
+        const int f2_lo = BATCH ? s_seg[3] : 0, n_items = BATCH ? n_own + s_seg[4] - f2_lo : n_own;
         C2 n0[2], n1[2], o0[2], o1[2];
         auto prefetch_slab = [&](int it, bool with_old) {
             const int f = it < n_own ? f_lo + it : f2_lo + (it - n_own), kxi = it < n_own ? kx : kx2;
@@ -548,7 +551,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
         PSTAMP(PT_RHO);
 #pragma unroll 1
         for (int it = 0; it < n_items; ++it) {
-            const bool own = it < n_own;
+            const bool own = !BATCH || it < n_own;
             const int f = own ? f_lo + it : f2_lo + (it - n_own), kxi = own ? kx : kx2;
             const C2 *msi = own ? ms : ms2;
             const T wkx = (kxi == 0 || 2 * kxi == P) ? (T)1 : (T)2;
@@ -655,10 +658,32 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
             if (rnd == 0) PSTAMP(PT_R_FFT1);
             if (rnd == 0) {
                 // scalars: alpha_k, mode coefficients (reduction items from the top warps down)
-                for (int item = NW - 1 - warp; item < F * NQ; item += NW) {
-                    const int f = item / NQ, qq = item - f * NQ;
-                    const double s = (qq == 0 || a.any_remove) ? warp_sum_cg160(a.part_s + ((size_t)f * NQ + qq) * Ph, Ph, lane) : 0.0;
-                    if (lane == 0) scal[f * SB + (qq == 0 ? SC_PQ : SC_HEAD + qq - 1)] = s;
+                // (four items per trip, all their loads in flight at once: at batch 16 a warp has 13 items and one L2 round
+                // trip per item cost 7.5 us)
+                constexpr int NLD = (Ph + 31) / 32, NB = BATCH ? 4 : 1;
+                for (int item0 = NW - 1 - warp; item0 < F * NQ; item0 += NB * NW) {
+                    double v[NB][NLD];
+#pragma unroll
+                    for (int j = 0; j < NB; ++j) {
+                        const int item = item0 + j * NW;
+                        const int f = item / NQ, qq = item - f * NQ;
+                        const bool on = item < F * NQ && (qq == 0 || a.any_remove);
+                        const double *src = a.part_s + ((size_t)f * NQ + qq) * Ph;
+#pragma unroll
+                        for (int m = 0; m < NLD; ++m) { const int i = lane + 32 * m; v[j][m] = (on && i < Ph) ? __ldcg(src + i) : 0.0; }
+                    }
+#pragma unroll
+                    for (int j = 0; j < NB; ++j) {
+                        const int item = item0 + j * NW;
+                        if (item < F * NQ) {
+                            const int f = item / NQ, qq = item - f * NQ;
+                            double t;
+                            if constexpr (NLD == 5) t = ((v[j][0] + v[j][1]) + (v[j][2] + v[j][3])) + v[j][4];     // the order warp_sum_cg160 used
+                            else { t = v[j][0]; for (int m = 1; m < NLD; ++m) t += v[j][m]; }
+                            const double s = warp_sum(t);
+                            if (lane == 0) scal[f * SB + (qq == 0 ? SC_PQ : SC_HEAD + qq - 1)] = s;
+                        }
+                    }
                 }
                 __syncthreads();
                 // alpha_k is recorded for the next phase C / the tail; every row unit derives alpha and its own mode
@@ -700,37 +725,57 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                 // loads and stores are LDS/STS resp. LDG/STG, not generic
                 auto update_rows = [&](T *ux, T *ur, T *up) {
                     constexpr int NX = (P / 2 + kGS) / kGS;              // columns per lane, n <= P/2 + 1
+                    constexpr int NH = BATCH ? (NX + 1) / 2 : 1;         // two halves: every load of a half is issued before its
+                                                                         // first store (a store between two loads serialises them:
+                                                                         // one L2 round trip per element with the rows in global memory)
 #pragma unroll
-                    for (int m = 0; m < NX; ++m) {
-                        const int xp = gl + m * kGS;
-                        if (xp < n) {
-                            const C2 z = bufA[xp];
-                            T nr[2] = {(T)0, (T)0};
+                    for (int h0 = 0; h0 < NX; h0 += NH) {
+                        T rv_[NH][2], pv_[NH][2], xv_[NH][2];
+#pragma unroll
+                        for (int mm = 0; mm < NH; ++mm) {
+                            const int m = h0 + mm, xp = gl + m * kGS;
 #pragma unroll
                             for (int row = 0; row < 2; ++row) {
-                                if ((vm >> (row * 16 + m)) & 1u) {
-                                    const T coord = ((q.comp ? (T)(q.y0 + row) : (T)xp) - half_n) * dd;
-                                    const T qp = (row ? -z.y : z.x) - (c0 + c2 * coord);
+                                rv_[mm][row] = pv_[mm][row] = xv_[mm][row] = (T)0;
+                                if (m < NX && xp < n && ((vm >> (row * 16 + m)) & 1u)) {
                                     const int idx = row * n + xp;
-                                    T rv;
-                                    if (pre) {                                   // warm start: r = b - M_s q, p = r
-                                        rv = ub[idx] - qp;
-                                        ur[idx] = rv; up[idx] = rv;
-                                    } else {
-                                        rv = ur[idx];
-                                        T pv = up[idx];
-                                        if (upd) { pv = rv + beta * pv; up[idx] = pv; }
-                                        if (step) {
-                                            ux[idx] += alpha * pv;
-                                            rv -= alpha * qp;
-                                            ur[idx] = rv;
-                                        }
-                                    }
-                                    rr += (double)rv * (double)rv;
-                                    nr[row] = rv;
+                                    if (pre) rv_[mm][row] = ub[idx];
+                                    else { rv_[mm][row] = ur[idx]; pv_[mm][row] = up[idx]; xv_[mm][row] = ux[idx]; }
                                 }
                             }
-                            bufA[xp] = mk<T>(nr[0], nr[1]);
+                        }
+#pragma unroll
+                        for (int mm = 0; mm < NH; ++mm) {
+                            const int m = h0 + mm, xp = gl + m * kGS;
+                            if (m < NX && xp < n) {
+                                const C2 z = bufA[xp];
+                                T nr[2] = {(T)0, (T)0};
+#pragma unroll
+                                for (int row = 0; row < 2; ++row) {
+                                    if ((vm >> (row * 16 + m)) & 1u) {
+                                        const T coord = ((q.comp ? (T)(q.y0 + row) : (T)xp) - half_n) * dd;
+                                        const T qp = (row ? -z.y : z.x) - (c0 + c2 * coord);
+                                        const int idx = row * n + xp;
+                                        T rv;
+                                        if (pre) {                                   // warm start: r = b - M_s q, p = r
+                                            rv = rv_[mm][row] - qp;
+                                            ur[idx] = rv; up[idx] = rv;
+                                        } else {
+                                            rv = rv_[mm][row];
+                                            T pv = pv_[mm][row];
+                                            if (upd) { pv = rv + beta * pv; up[idx] = pv; }
+                                            if (step) {
+                                                ux[idx] = xv_[mm][row] + alpha * pv;
+                                                rv -= alpha * qp;
+                                                ur[idx] = rv;
+                                            }
+                                        }
+                                        rr += (double)rv * (double)rv;
+                                        nr[row] = rv;
+                                    }
+                                }
+                                bufA[xp] = mk<T>(nr[0], nr[1]);
+                            }
                         }
                     }
                 };
