@@ -32,6 +32,12 @@ int tomo_host_generator_spectrum(const double *gen, int n_out, int n_in, int P, 
 /* D_phi(r) of Eq.53 (L619) for count separations r [m]. */
 int tomo_host_structure_function(const double *r, int count, double r0, double L0, double *out);
 
+/* Work table of the persistent solver's batch path: how the Ph x n_frames slab passes of one CG iteration (one k_x slab of
+ * all channels of one frame: y-FFTs + the per-frequency block product, Eq.22 / Eq.30) are dealt to n_ctas CTAs.  CTA b
+ * owns slab b % Ph with the other CTAs of that residue; CTAs above the average hand frames to CTAs below it (one helped
+ * slab per CTA).  seg_out: host int [n_ctas][8] = {own f_lo, own f_hi, helped k_x, helped f_lo, helped f_hi, 0, 0, 0}. */
+int tomo_host_slab_segments(int Ph, int n_frames, int n_ctas, int *seg_out);
+
 #ifdef __cplusplus
 }
 #endif

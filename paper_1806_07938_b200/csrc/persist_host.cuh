@@ -22,7 +22,7 @@ struct PersistState {
     double *d_part_r = nullptr, *d_part_s = nullptr, *d_part_i = nullptr;
     int G = 0, nq_m = 1, NQ = 0, SB = 0, any_remove = 0, spec_smem = 0, vec_smem = 0;
     int off_ms = 0, off_work = 0, off_red = 0, off_scal = 0, off_tab = 0, off_upart = 0, off_vm = 0, off_vec = 0, off_spec = 0, off_ptab = 0, off_unit = 0, ngs = 2;
-    int off_ms2 = 0;
+    int off_ms2 = 0, fb = 1;
     size_t smem = 0;
     bool attr_set = false, attr_set_batch = false;
     int *d_seg = nullptr;        // [F_max + 1][sms][8] slab segment tables, one per frame count (slab_segments)
@@ -68,7 +68,7 @@ static int persist_launch(tomo_plan *pl, cudaStream_t st, const PLaunch &L) {
     a.off_ms = ps->off_ms; a.off_work = ps->off_work; a.off_red = ps->off_red; a.off_scal = ps->off_scal;
     a.off_tab = ps->off_tab; a.off_upart = ps->off_upart; a.off_vm = ps->off_vm; a.off_vec = ps->off_vec;
     a.off_spec = ps->off_spec; a.off_ptab = ps->off_ptab; a.off_unit = ps->off_unit; a.ngs = ps->ngs;
-    a.off_ms2 = ps->off_ms2;
+    a.off_ms2 = ps->off_ms2; a.fb = ps->fb;
     if (!ps->seg_ready[L.F]) {
         std::vector<int> seg;
         slab_segments(m.Ph, L.F, a.G, seg);

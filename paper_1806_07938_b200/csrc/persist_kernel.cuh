@@ -64,6 +64,7 @@ template <typename T, typename S> struct PArgs {
     int off_ms, off_work, off_red, off_scal, off_tab, off_upart, off_vm, off_vec, off_spec, off_ptab, off_unit;
     int ngs;                     // row-unit buffer slots in shared memory = row units processed per round
     int off_ms2;                 // mask spectra of the helped slab
+    int fb;                      // batch instance: frames per slab pass (1 or 2: two frames share the four FFT passes)
     const int *seg;              // [G][8] slab work of a CTA: own frames [0],[1]; helped slab k_x [2], frames [3],[4] (balance)
     const float *s_in;           // [F][C][nv] slopes (COLD/WARM)
     const float *x0;             // [F][C][nv] warm start (WARM)
@@ -306,7 +307,9 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
     S2 *sspec = reinterpret_cast<S2 *>(smem_raw + a.off_spec);
     PairRef *ptab = reinterpret_cast<PairRef *>(smem_raw + a.off_ptab);
     UnitRec *s_unit = reinterpret_cast<UnitRec *>(smem_raw + a.off_unit);
-    C2 *Ubuf = work, *Vbuf = work + (size_t)C * LD;
+    const int FB = BATCH ? a.fb : 1;                           // frames per slab pass
+    const int red_sz = (min(kPWarps / ((P + 31) >> 5), C) + 2 * C) * P;      // partial sums of one frame (mac_slab)
+    C2 *Ubuf = work, *Vbuf = work + (size_t)FB * C * LD;      // [frame of the pass][c][LD] each
     const int NGS = a.ngs;
     C2 *bufA = work + (size_t)(gs < NGS ? gs : 0) * (P + LD), *bufB = bufA + P;   // row unit: natural [P], pass-1 result [LD]
     unsigned epoch = 0;
@@ -325,13 +328,15 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
     __syncthreads();
     const bool has_slab = (s_seg[1] - s_seg[0]) + (s_seg[4] - s_seg[3]) > 0;
     // slab thread maps
-    const bool it1 = tid < C * B, it2 = tid < C * A;
     const int c1 = tid / B, j2s = tid - c1 * B;      // pass 1: (channel, j2)
     const int c2s = tid / A, k1s = tid - c2s * A;    // pass 2: (channel, k1)
-    const int w_busy = (C * B + 31) >> 5;            // warps that carry slab pass-1 items
-    const int n_free = (NW - w_busy) > 0 ? NW - w_busy : NW;
     // ---- row units of this CTA: ut = b + i G, i < nu; NGS of them per round, unit i0 + gs by the 16 lanes of group gs
-    const int nu = (b < F * U) ? (F * U - b + G - 1) / G : 0;
+    // single frame: strided (unit b + i G); batch: a contiguous chunk, so that a CTA's units belong to one or two frames and
+    // it needs the modal sums of those frames only
+    const int u_chunk = (F * U + G - 1) / G;
+    const int u_base = BATCH ? b * u_chunk : b, u_stride = BATCH ? 1 : G;
+    const int nu = BATCH ? max(0, min(u_chunk, F * U - u_base)) : ((b < F * U) ? (F * U - b + G - 1) / G : 0);
+    const int fu_lo = BATCH ? min(u_base, F * U - 1) / U : 0, fu_n = BATCH ? (nu > 0 ? (u_base + nu - 1) / U - fu_lo + 1 : 0) : F;
     const int n_rounds = nu > 0 ? (nu + NGS - 1) / NGS : 1;
 
     for (int i = tid; i < P; i += kPThreads) tw[i] = a.tw[i];
@@ -360,7 +365,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
     for (int i = tid; i < nu * kGS; i += kPThreads) s_vm[i] = 0u;
     for (int i = tid; i < (nu > 0 ? nu : 1); i += kPThreads) {
         UnitRec u;
-        const int ut = min(b + i * G, F * U - 1);
+        const int ut = min(u_base + i * u_stride, F * U - 1);
         u.f = ut / U;
         const int uu = ut - u.f * U;
         u.c = uu / npairs; u.j = uu - u.c * npairs;
@@ -446,7 +451,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
         if (a.any_remove && a.mode != PM_STATE) {
             t0 = group_sum(t0); t1 = group_sum(t1);
             if (act && gl == 0) {
-                const int u = (b + i * G) - q.f * U;
+                const int u = (u_base + i * u_stride) - q.f * U;
                 a.part_i[((size_t)q.f * U + u) * 2] = t0; a.part_i[((size_t)q.f * U + u) * 2 + 1] = t1;
             }
         }
@@ -491,7 +496,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
             }
         }
         rr = group_sum(rr);
-        if (act && gl == 0) a.part_r[b + i * G] = rr;                   // [f][unit]: unit index b + i G = f U + u
+        if (act && gl == 0) a.part_r[u_base + i * u_stride] = rr;       // [f][unit]: unit index = f U + u
         fwd_unit(q, act);
     }
     GRID_SYNC();
@@ -550,81 +555,101 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
         __syncthreads();
         PSTAMP(PT_RHO);
 #pragma unroll 1
-        for (int it = 0; it < n_items; ++it) {
+        for (int it = 0; it < n_items;) {
             const bool own = !BATCH || it < n_own;
-            const int f = own ? f_lo + it : f2_lo + (it - n_own), kxi = own ? kx : kx2;
+            // batch: two consecutive frames of the same slab go through one pass together (the FFT passes are latency-bound
+            // with 192 / 120 of the 512 threads busy: the second frame rides along)
+            const int nf = (BATCH && FB == 2 && it + 1 < n_items && (it + 1 < n_own || it >= n_own)) ? 2 : 1;
+            const int f0 = own ? f_lo + it : f2_lo + (it - n_own), kxi = own ? kx : kx2;
             const C2 *msi = own ? ms : ms2;
             const T wkx = (kxi == 0 || 2 * kxi == P) ? (T)1 : (T)2;
-            const double *sc = scal + f * SB;
-            const bool upd = !pre && sc[SC_UPD] != 0.0;
-            const T beta = (T)sc[SC_BETA];
-            C2 *t1p = a.T1p + ((size_t)f * Ph + kxi) * C * npad;
-            if (it != 0) prefetch_slab(it, !take_new);
+            if (!BATCH && it != 0) prefetch_slab(it, !take_new);     // (batch instance: issued before the previous pass's T2 store)
             // p~rows = r~rows + beta p~rows_old on rows 0..n-1 -> Vbuf[c][y] (the padding rows n..P-1 are never stored)
+            for (int fr = 0; fr < nf; ++fr) {
+                const int f = f0 + fr;
+                const double *sc = scal + f * SB;
+                const bool upd = !pre && sc[SC_UPD] != 0.0;
+                const T beta = (T)sc[SC_BETA];
+                C2 *t1p = a.T1p + ((size_t)f * Ph + kxi) * C * npad;
+                C2 *Vf = Vbuf + (size_t)fr * C * LD;
+                if (fr) prefetch_slab(it + fr, !take_new);
 #pragma unroll
-            for (int m = 0; m < 2; ++m) {
-                const int e2 = tid + m * kPThreads;
-                if (e2 < n_t1) {
-                    C2 v0, v1;
-                    if (take_new) { v0 = n0[m]; v1 = n1[m]; }
-                    else if (upd) { v0 = mk<T>(n0[m].x + beta * o0[m].x, n0[m].y + beta * o0[m].y); v1 = mk<T>(n1[m].x + beta * o1[m].x, n1[m].y + beta * o1[m].y); }
-                    else { v0 = o0[m]; v1 = o1[m]; }
-                    if (take_new || upd) st_pair(t1p + 2 * e2, v0, v1);
-                    Vbuf[voff[m]] = v0;
-                    if (vtwo[m]) Vbuf[voff[m] + 1] = v1;
+                for (int m = 0; m < 2; ++m) {
+                    const int e2 = tid + m * kPThreads;
+                    if (e2 < n_t1) {
+                        C2 v0, v1;
+                        if (take_new) { v0 = n0[m]; v1 = n1[m]; }
+                        else if (upd) { v0 = mk<T>(n0[m].x + beta * o0[m].x, n0[m].y + beta * o0[m].y); v1 = mk<T>(n1[m].x + beta * o1[m].x, n1[m].y + beta * o1[m].y); }
+                        else { v0 = o0[m]; v1 = o1[m]; }
+                        if (take_new || upd) st_pair(t1p + 2 * e2, v0, v1);
+                        Vf[voff[m]] = v0;
+                        if (vtwo[m]) Vf[voff[m] + 1] = v1;
+                    }
                 }
             }
             __syncthreads();
             PSTAMP(PT_BUILD);
-            // forward y-FFT: pass 1 Vbuf -> Ubuf, pass 2 Ubuf -> Vbuf (natural k_y)
-            if (it1) dft_pass<T, A, true>(Vbuf + c1 * LD + j2s, B, (n - j2s + B - 1) / B, Ubuf + c1 * LD + j2s, B + 1, tw, j2s);
+            // forward y-FFT of the nf * C columns: pass 1 Vbuf -> Ubuf, pass 2 Ubuf -> Vbuf (natural k_y)
+            const bool p1 = tid < nf * C * B, p2 = tid < nf * C * A;
+            if (p1) dft_pass<T, A, true>(Vbuf + c1 * LD + j2s, B, (n - j2s + B - 1) / B, Ubuf + c1 * LD + j2s, B + 1, tw, j2s);
             __syncthreads();
-            if (it2) dft_pass<T, B, false>(Ubuf + c2s * LD + k1s * (B + 1), 1, B, Vbuf + c2s * LD + k1s, A, tw, 0);
+            if (p2) dft_pass<T, B, false>(Ubuf + c2s * LD + k1s * (B + 1), 1, B, Vbuf + c2s * LD + k1s, A, tw, 0);
             __syncthreads();
             PSTAMP(PT_FFT);
-#define TOMO_MAC(CT_, SP_) mac_slab<T, S, CT_, P>(Vbuf, Ubuf, LD, SP_, ptab, msi, s_s2c, C, P, a.nq_m, a.any_remove, red, warp, lane)
+#define TOMO_MAC(CT_, SP_) mac_slab<T, S, CT_, P>(Vbuf + (size_t)fr * C * LD, Ubuf + (size_t)fr * C * LD, LD, SP_, ptab, msi, s_s2c, C, P, a.nq_m, a.any_remove, red + fr * red_sz, warp, lane)
 #define TOMO_MAC_SWITCH(SP_)                                                               \
     switch (C) {                                                                           \
         case 4: TOMO_MAC(4, SP_); break;   case 6: TOMO_MAC(6, SP_); break;                \
         case 8: TOMO_MAC(8, SP_); break;   case 12: TOMO_MAC(12, SP_); break;              \
         case 16: TOMO_MAC(16, SP_); break; default: TOMO_MAC(0, SP_); break;               \
     }
-            if (a.spec_smem && own) { TOMO_MAC_SWITCH(sspec) } else { const S2 *gsp = a.spec + (size_t)kxi * a.n_pair * P; TOMO_MAC_SWITCH(gsp) }     // shared vs global loads
+#pragma unroll 1
+            for (int fr = 0; fr < nf; ++fr) {
+                if (a.spec_smem && own) { TOMO_MAC_SWITCH(sspec) } else { const S2 *gsp = a.spec + (size_t)kxi * a.n_pair * P; TOMO_MAC_SWITCH(gsp) }     // shared vs global loads
+            }
 #undef TOMO_MAC_SWITCH
 #undef TOMO_MAC
             __syncthreads();
             PSTAMP(PT_MAC);
             // inverse y-FFT as a forward transform of conj(y~): pass 1 Ubuf -> Vbuf; the warps without pass-1 items
             // reduce the slab partials meanwhile
-            if (it1) dft_pass<T, A, true>(Ubuf + c1 * LD + j2s, B, A, Vbuf + c1 * LD + j2s, B + 1, tw, j2s);
+            if (p1) dft_pass<T, A, true>(Ubuf + c1 * LD + j2s, B, A, Vbuf + c1 * LD + j2s, B + 1, tw, j2s);
             {
                 const int WPG = (P + 31) >> 5, Goc = min(NW / WPG, C);
+                // (batch: every warp takes its share once its pass-1 column is done; with two frames only 4 warps are free)
+                const int wb = (nf * C * B + 31) >> 5, nfree = (!BATCH && (NW - wb) > 0) ? NW - wb : NW;
                 const int slot = NW - 1 - warp;             // free warps are the top ones
-                if (slot < n_free) {
-                    for (int tq = slot; tq < NQ; tq += n_free) {
+                if (slot < nfree) {
+                    for (int tq = slot; tq < nf * NQ; tq += nfree) {
+                        const int fr = tq / NQ, q1 = tq - fr * NQ;
+                        const T *rd = red + fr * red_sz;
                         double s = 0.0;
-                        if (tq == 0) s = warp_sum_red<T>(red, Goc * P, lane);
-                        else if (a.any_remove) s = warp_sum_red<T>(red + (Goc + tq - 1) * P, P, lane);
-                        if (lane == 0) a.part_s[((size_t)f * NQ + tq) * Ph + kxi] = (double)wkx * s;
+                        if (q1 == 0) s = warp_sum_red<T>(rd, Goc * P, lane);
+                        else if (a.any_remove) s = warp_sum_red<T>(rd + (Goc + q1 - 1) * P, P, lane);
+                        if (lane == 0) a.part_s[((size_t)(f0 + fr) * NQ + q1) * Ph + kxi] = (double)wkx * s;
                     }
                 }
             }
             __syncthreads();
-            if (it2) dft_pass<T, B, false>(Vbuf + c2s * LD + k1s * (B + 1), 1, B, Ubuf + c2s * LD + k1s, A, tw, 0);
+            if (p2) dft_pass<T, B, false>(Vbuf + c2s * LD + k1s * (B + 1), 1, B, Ubuf + c2s * LD + k1s, A, tw, 0);
             __syncthreads();
+            // batch: the T1 / T1p loads of the next pass fly during this pass's T2 store
+            if (BATCH && it + nf < n_items) prefetch_slab(it + nf, !take_new);
             // image rows y < n (conjugate back) -> T2[c][y / 2][kx][y & 1]
-            {
-                C2 *dst = a.T2 + (size_t)f * C * npairs * Ph * 2 + (size_t)kxi * 2;
+            for (int fr = 0; fr < nf; ++fr) {
+                C2 *dst = a.T2 + (size_t)(f0 + fr) * C * npairs * Ph * 2 + (size_t)kxi * 2;
+                const C2 *Uf = Ubuf + (size_t)fr * C * LD;
 #pragma unroll
                 for (int m = 0; m < 2; ++m) {
                     const int e = tid + m * kPThreads;
                     if (e < n_t1) {
-                        const C2 u0 = Ubuf[voff[m]], u1 = vtwo[m] ? Ubuf[voff[m] + 1] : mk<T>((T)0, (T)0);
+                        const C2 u0 = Uf[voff[m]], u1 = vtwo[m] ? Uf[voff[m] + 1] : mk<T>((T)0, (T)0);
                         st_pair(dst + (size_t)e * Ph * 2, mk<T>(u0.x, -u0.y), mk<T>(u1.x, -u1.y));
                     }
                 }
             }
             __syncthreads();
+            it += nf;
         }
         PSTAMP(PT_INV);
         GRID_SYNC();
@@ -660,14 +685,23 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                 // scalars: alpha_k, mode coefficients (reduction items from the top warps down)
                 // (four items per trip, all their loads in flight at once: at batch 16 a warp has 13 items and one L2 round
                 // trip per item cost 7.5 us)
+                // items: p.q of every frame (alpha of the frames of the CTA's slab passes), then the modal sums of the frames
+                // of its row units (batch: one or two frames; single frame: item = qq)
                 constexpr int NLD = (Ph + 31) / 32, NB = BATCH ? 4 : 1;
-                for (int item0 = NW - 1 - warp; item0 < F * NQ; item0 += NB * NW) {
+                const int n_sc = BATCH ? F + fu_n * (NQ - 1) : F * NQ;
+                auto sc_item = [&](int item, int &f, int &qq) {
+                    if (!BATCH) { f = item / NQ; qq = item - f * NQ; }
+                    else if (item < F) { f = item; qq = 0; }
+                    else { const int r = item - F; f = fu_lo + r / (NQ - 1); qq = 1 + r % (NQ - 1); }
+                };
+                for (int item0 = NW - 1 - warp; item0 < n_sc; item0 += NB * NW) {
                     double v[NB][NLD];
 #pragma unroll
                     for (int j = 0; j < NB; ++j) {
                         const int item = item0 + j * NW;
-                        const int f = item / NQ, qq = item - f * NQ;
-                        const bool on = item < F * NQ && (qq == 0 || a.any_remove);
+                        int f = 0, qq = 0;
+                        if (item < n_sc) sc_item(item, f, qq);
+                        const bool on = item < n_sc && (qq == 0 || a.any_remove);
                         const double *src = a.part_s + ((size_t)f * NQ + qq) * Ph;
 #pragma unroll
                         for (int m = 0; m < NLD; ++m) { const int i = lane + 32 * m; v[j][m] = (on && i < Ph) ? __ldcg(src + i) : 0.0; }
@@ -675,8 +709,9 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
 #pragma unroll
                     for (int j = 0; j < NB; ++j) {
                         const int item = item0 + j * NW;
-                        if (item < F * NQ) {
-                            const int f = item / NQ, qq = item - f * NQ;
+                        if (item < n_sc) {
+                            int f, qq;
+                            sc_item(item, f, qq);
                             double t;
                             if constexpr (NLD == 5) t = ((v[j][0] + v[j][1]) + (v[j][2] + v[j][3])) + v[j][4];     // the order warp_sum_cg160 used
                             else { t = v[j][0]; for (int m = 1; m < NLD; ++m) t += v[j][m]; }
@@ -788,7 +823,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                 }
             }
             rr = group_sum(rr);
-            if (act && gl == 0) a.part_r[b + i * G] = rr;                   // [f][unit]: unit index b + i G = f U + u
+            if (act && gl == 0) a.part_r[u_base + i * u_stride] = rr;       // [f][unit]: unit index = f U + u
             if (rnd == 0) PSTAMP(PT_R_UPD);
             fwd_unit(q, act);
             if (rnd == 0) PSTAMP(PT_R_FFT2);

@@ -9,6 +9,7 @@
 #include <vector>
 
 #include "persist_host.cuh"
+#include "tomo_host.h"
 #include "tomo_kernels_cos.cuh"
 
 namespace tomo {
@@ -77,6 +78,18 @@ void slab_segments(int Ph, int F, int G, std::vector<int> &seg) {
     }
 }
 
+}  // namespace tomo
+
+extern "C" int tomo_host_slab_segments(int Ph, int n_frames, int n_ctas, int *seg_out) {
+    if (Ph < 1 || n_frames < 1 || n_ctas < Ph || !seg_out) { tomo::set_error("bad arguments"); return TOMO_EINVAL; }
+    std::vector<int> seg;
+    tomo::slab_segments(Ph, n_frames, n_ctas, seg);
+    std::memcpy(seg_out, seg.data(), seg.size() * sizeof(int));
+    return TOMO_OK;
+}
+
+namespace tomo {
+
 static int persist_prepare(tomo_plan *pl) {
     if (pl->persist) return TOMO_OK;
     const HostModel &m = pl->m;
@@ -115,16 +128,19 @@ static int persist_prepare(tomo_plan *pl) {
     const int WPG = (m.P + 31) / 32, Goc = std::min(kPWarps / WPG, m.C);
     const int maxu = (F * U + ps->G - 1) / ps->G;
     const size_t LD = (size_t)fa * (fb + 1);
-    ps->ngs = std::min(kPThreads / kGS, (maxu + 1) & ~1);
+    // row-unit slots per round: as few rounds as 32 groups allow, then as few slots as those rounds need
+    const int rounds = std::max(1, (maxu + kPThreads / kGS - 1) / (kPThreads / kGS));
+    ps->ngs = std::min(kPThreads / kGS, (((maxu + rounds - 1) / rounds) + 1) & ~1);
+    ps->fb = (F > 1 && 2 * m.C * fb <= kPThreads) ? 2 : 1;      // frames per slab pass of the batch instance
     size_t off = (size_t)m.P * 2 * E;
     ps->off_ms = (int)(off = align16(off));
     off += (size_t)ps->nq_m * m.P * 2 * E;
     ps->off_ms2 = (int)(off = align16(off));
     off += (size_t)ps->nq_m * m.P * 2 * E + 32;      // + the CTA's row of the slab segment table
     ps->off_work = (int)(off = align16(off));
-    off += std::max((size_t)2 * m.C * LD, (size_t)ps->ngs * (m.P + LD)) * 2 * E;
+    off += std::max((size_t)2 * ps->fb * m.C * LD, (size_t)ps->ngs * (m.P + LD)) * 2 * E;
     ps->off_red = (int)(off = align16(off));
-    off += (size_t)(Goc + 2 * m.C) * m.P * E;
+    off += (size_t)ps->fb * (Goc + 2 * m.C) * m.P * E;
     ps->off_scal = (int)(off = align16(off));
     off += (size_t)F * ps->SB * sizeof(double);
     ps->off_tab = (int)(off = align16(off));

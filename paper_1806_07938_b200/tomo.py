@@ -27,7 +27,7 @@ EXPORTS = (
     "tomo_get_sizes", "tomo_get_valid_index", "tomo_get_noise",
     "tomo_get_residuals", "tomo_get_stats", "tomo_plan_destroy", "tomo_last_error",
     "tomo_host_sizes", "tomo_host_css_generators", "tomo_host_cos_generators", "tomo_host_generator_spectrum",
-    "tomo_host_structure_function",
+    "tomo_host_structure_function", "tomo_host_slab_segments",
 )
 
 
@@ -105,6 +105,7 @@ def load(build_if_missing: bool = True):
                                              C.c_int, dp]
     lib.tomo_host_generator_spectrum.argtypes = [dp, C.c_int, C.c_int, C.c_int, dp]
     lib.tomo_host_structure_function.argtypes = [dp, C.c_int, C.c_double, C.c_double, dp]
+    lib.tomo_host_slab_segments.argtypes = [C.c_int, C.c_int, C.c_int, ip]
     _lib = lib
     return lib
 
@@ -179,6 +180,13 @@ def host_structure_function(r, r0: float, L0: float) -> np.ndarray:
     out = np.empty_like(rr)
     _check(lib.tomo_host_structure_function(_dp(rr), rr.size, r0, L0, _dp(out)))
     return out.reshape(np.shape(r))
+
+
+def host_slab_segments(Ph: int, n_frames: int, n_ctas: int) -> np.ndarray:
+    lib = load()
+    out = np.zeros((n_ctas, 8), dtype=np.int32)
+    _check(lib.tomo_host_slab_segments(Ph, n_frames, n_ctas, out.ctypes.data_as(C.POINTER(C.c_int))))
+    return out
 
 
 # ------------------------------------------------------------------------------------------------ the plan

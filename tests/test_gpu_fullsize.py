@@ -91,7 +91,7 @@ def test_sweep_sizes_product_on_sampled_outputs_from_positions(n):
 
 
 def test_cfg3_solve_and_projection_against_the_matrix_free_oracle():
-    """Whole product, 12 free-running CG iterations (below the fp32 horizon) and the projection at cfg3."""
+    """Whole product, 12 free-running CG and MINRES iterations (below the fp32 horizon) and the projection at cfg3."""
     cfg = get_config("cfg3")
     osys = OracleSystem(cfg, dense=False)
     _build_generators_in_parallel(osys)
@@ -119,6 +119,16 @@ def test_cfg3_solve_and_projection_against_the_matrix_free_oracle():
     pl.apply_cos(dev(x_or), d_w)
     torch.cuda.synchronize()
     assert rel(d_w.cpu().numpy(), osys.reconstruct(f32(x_or), 0)) <= 1e-4
+    # M-c at full size: 12 free-running MINRES iterations (tomo_solve_minres) against the oracle's MINRES on the same
+    # matrix-free operator; the residual never increases and stays below CG's
+    pl.solve_minres(dev(s), d_w, 1, n_it)
+    pl.get_zeta(d_z)
+    torch.cuda.synchronize()
+    xm_or, hm_or = osys.solve_minres(s, n_it)
+    hm_gpu = pl.residuals(1, n_it)[0]
+    assert np.abs(hm_gpu / hm_or - 1.0).max() <= 1e-3
+    assert rel(d_z.cpu().numpy(), xm_or) <= 1e-3
+    assert np.all(np.diff(hm_gpu) <= 0) and np.all(hm_gpu <= h_gpu * (1 + 1e-5))
     pl.close()
 
 

@@ -90,3 +90,28 @@ def test_generator_spectrum_is_the_scaled_rfft2_of_the_embedding(P):
     sp = tomo.host_generator_spectrum(g, n_out, n_in, P)
     ref = np.fft.rfft2(tz.embed_generator(g, n_in, n_out, P)) / P ** 2      # [ky][kx]
     np.testing.assert_allclose(sp, ref.T, atol=1e-14 * np.abs(ref).max() * P)
+
+
+def test_slab_segments_cover_every_pass_once_and_balance():
+    """Host table of the persistent solver's batch path (include/tomo_host.h: tomo_host_slab_segments)."""
+    for Ph, F, G in [(81, 1, 148), (81, 2, 148), (81, 3, 148), (81, 4, 148), (81, 16, 148), (81, 5, 148), (97, 16, 148),
+                     (129, 16, 148), (129, 7, 148), (65, 16, 148), (9, 16, 148), (21, 16, 148), (11, 5, 148), (81, 16, 81)]:
+        seg = tomo.host_slab_segments(Ph, F, G)
+        seen = np.zeros((Ph, F), dtype=int)
+        load = np.zeros(G, dtype=int)
+        for b in range(G):
+            f_lo, f_hi, kx2, g_lo, g_hi = (int(v) for v in seg[b, :5])
+            assert 0 <= f_lo <= f_hi <= F and 0 <= g_lo <= g_hi <= F and 0 <= kx2 < Ph
+            seen[b % Ph, f_lo:f_hi] += 1
+            seen[kx2, g_lo:g_hi] += 1
+            load[b] = (f_hi - f_lo) + (g_hi - g_lo)
+            if g_hi > g_lo:
+                assert kx2 != b % Ph                                  # a helped slab is somebody else's
+        assert np.all(seen == 1), (Ph, F, G)                          # every (k_x, frame) pass exactly once
+        target = -(-Ph * F // G)
+        unbalanced = max(-(-F // ((G - 1 - kx) // Ph + 1)) for kx in range(Ph))
+        assert load.max() <= unbalanced                               # never worse than without helpers
+        if (Ph, F, G) in [(81, 16, 148), (81, 4, 148), (81, 3, 148), (97, 16, 148)]:
+            assert load.max() == target < unbalanced, (Ph, F, G, load.max(), target)
+        if F == 1:
+            assert load.max() == 1 and not np.any(seg[:, 4] > seg[:, 3])
