@@ -296,6 +296,24 @@ def main():
                         "peak_TFLOPs": fp32_peak / 1e12, "frac": B * n_iter * f_iter / (k_ms * 1e-3) / fp32_peak},
                 "state": ("one cooperative launch per solve; spectra pinned in shared memory, exchange buffers L2-resident: "
                           "latency-bound at batch 1 (two grid barriers per iteration), see DESIGN.md 6")}
+    # L2 roofline (north_star: "... and over L2 bandwidth where the spectra are L2-resident"): the device's L2 -> SM read
+    # bandwidth and plain FMA rate measured by the library's own kernels in this run (tomo_measure_device)
+    dev_meas = tomo.measure_device(0, 5, stream=stream)
+    npairs_rows = (n + 1) // 2
+    exch = Ph * C * 2 * npairs_rows * 2 * E                       # one row <-> column exchange buffer of one frame
+    if args.solver == "persistent":
+        # per frame-iteration through L2: T1 written + read, T1p read + written, T2 written + read (spectra sit in shared memory)
+        l2_bytes_iter = B * 6 * exch
+        l2_what = "T1, T1p, T2 exchange buffers: 6 passes per frame-iteration (spectra pinned in shared memory)"
+    else:
+        l2_bytes_iter = spectra * B + B * 4 * tbuf + B * 9 * Ns * E     # k_cols re-reads the spectra per (k_x, frame) CTA
+        l2_what = "spectra per frame + 4 exchange passes + CG vector passes"
+    l2_roof = {"peak_GBps_measured": dev_meas["l2_read_GBps"], "bytes_per_iteration": l2_bytes_iter, "what": l2_what,
+               "achieved_GBps": l2_bytes_iter / (us_iter * 1e-6) / 1e9,
+               "frac": l2_bytes_iter / (us_iter * 1e-6) / 1e9 / max(dev_meas["l2_read_GBps"], 1e-9),
+               "b_iter_over_l2_peak_us": b_iter / max(dev_meas["l2_read_GBps"], 1e-9) / 1e3,
+               "fp32_TFLOPs_measured": dev_meas["fp32_TFLOPs"],
+               "f_iter_frac_of_measured_fp32": B * f_iter / (us_iter * 1e-6) / 1e12 / max(dev_meas["fp32_TFLOPs"], 1e-9)}
     iter_roof = {"b_iter_bytes": b_iter, "us_per_iteration": us_iter, "achieved_GBps": b_iter / (us_iter * 1e-6) / 1e9,
                  "frac_of_hbm_peak": b_iter / (us_iter * 1e-6) / 1e9 / hbm}
 
@@ -309,7 +327,7 @@ def main():
                        "l2": "flushed (256 MiB write) before every timed step"},
             "us_per_cg_iteration": us_iter, "ms_per_step_n_iter0": ms_step0, "ms_per_step_l2_warm": ms_step_warm,
             "reconstructions_per_s_l2_warm": world * B * 1e3 / ms_step_warm,
-            "iteration_roofline": iter_roof, "roofline": roof,
+            "iteration_roofline": iter_roof, "l2_roofline": l2_roof, "roofline": roof,
             "e2e": {"value": world * B * 1e3 / e2e_ms, "unit": "reconstructions/s", "ms_per_step": e2e_ms,
                     "h2d_bytes_per_step": int(h_slopes.numel() * 4), "d2h_bytes_per_step": int(out_h.numel() * 4)},
             "gpu_launches": launches * args.steps, "launches_per_step": launches, "clocks": clocks,

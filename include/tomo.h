@@ -168,6 +168,14 @@ int tomo_time_phases(tomo_plan *plan, int n_frames, int n_iter, float *us_out, v
 int tomo_time_solver(tomo_plan *plan, const float *slopes, int n_frames, int n_iter, int reps, float *ms_out,
                      void *cuda_stream);
 
+/* Measurement aid (bench.py "l2_roofline", north_star: "... and over L2 bandwidth where the spectra are L2-resident"): the
+ * device's L2 -> SM read bandwidth and its plain fp32 FMA rate, measured by two small kernels of this library on
+ * `cuda_stream` (synchronises the stream).  The bandwidth kernel sweeps an L2-resident buffer of `l2_bytes` (0 = 64 MiB;
+ * keep it under the L2 size) `reps` times with 16-byte `ld.global.cg` loads from 148 x 8 CTAs and returns the best
+ * repetition; the FMA kernel runs independent FFMA chains on every SM.  out (host fp32 [2]) = {L2 read GB/s, fp32 TFLOP/s}.
+ * Needs no plan.  Returns TOMO_ECUDA without a device. */
+int tomo_measure_device(long long l2_bytes, int reps, float *out, void *cuda_stream);
+
 /* Sizes fixed at plan creation; any pointer may be NULL. */
 int tomo_get_sizes(const tomo_plan *plan, int *n_vs, int *n_vphi, int *slopes_len, int *wavefront_len,
                    int *pad, int *pad_os, int *n_prime);

@@ -797,6 +797,86 @@ extern "C" int tomo_time_solver(tomo_plan *pl, const float *slopes, int n_frames
     return time_solver_persistent(pl, slopes, n_frames, n_iter, reps, ms_out, (cudaStream_t)cuda_stream);
 }
 
+// ---- measurement aid: L2 read bandwidth and fp32 FMA rate of the device (tomo_measure_device)
+namespace tomo {
+__global__ void __launch_bounds__(256) k_l2_sweep(const float4 *buf, size_t n4, int sweeps, float *sink) {
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (int s = 0; s < sweeps; ++s)
+        for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += 4 * stride) {
+            // four independent 16-byte L2 loads in flight per thread
+            const float4 a = __ldcg(buf + i);
+            const float4 b = (i + stride < n4) ? __ldcg(buf + i + stride) : make_float4(0.f, 0.f, 0.f, 0.f);
+            const float4 c = (i + 2 * stride < n4) ? __ldcg(buf + i + 2 * stride) : make_float4(0.f, 0.f, 0.f, 0.f);
+            const float4 d = (i + 3 * stride < n4) ? __ldcg(buf + i + 3 * stride) : make_float4(0.f, 0.f, 0.f, 0.f);
+            acc.x += a.x + b.x + c.x + d.x; acc.y += a.y + b.y + c.y + d.y;
+            acc.z += a.z + b.z + c.z + d.z; acc.w += a.w + b.w + c.w + d.w;
+        }
+    if (acc.x + acc.y + acc.z + acc.w == 12345.678f) sink[0] = acc.x;      // keeps the loads alive
+}
+__global__ void __launch_bounds__(256) k_fma_rate(int iters, float *sink) {
+    float a[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) a[j] = 1.0f + 1e-3f * (threadIdx.x + j);
+    const float m = 0.999f, c = 1e-3f;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) a[j] = fmaf(a[j], m, c);
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) s += a[j];
+    if (s == 12345.678f) sink[0] = s;
+}
+}  // namespace tomo
+
+extern "C" int tomo_measure_device(long long l2_bytes, int reps, float *out, void *cuda_stream) {
+    if (!out || reps < 1 || reps > 1000 || l2_bytes < 0) { set_error("bad arguments"); return TOMO_EINVAL; }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { set_error("no CUDA device: libtomo_b200 has no CPU fallback"); return TOMO_ECUDA; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, sms = 0;
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const size_t bytes = l2_bytes ? (size_t)l2_bytes : ((size_t)64 << 20);
+    const size_t n4 = bytes / 16;
+    float4 *buf = nullptr;
+    float *sink = nullptr;
+    CK(cudaMalloc(&buf, n4 * 16));
+    CK(cudaMalloc(&sink, 16));
+    CK(cudaMemsetAsync(buf, 0, n4 * 16, st));
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int sweeps = 20;
+    float best_bw = 0.f, best_fl = 0.f;
+    k_l2_sweep<<<sms * 8, 256, 0, st>>>(buf, n4, 2, sink);             // warm: the buffer becomes L2-resident
+    for (int r = 0; r < reps; ++r) {
+        cudaEventRecord(e0, st);
+        k_l2_sweep<<<sms * 8, 256, 0, st>>>(buf, n4, sweeps, sink);
+        cudaEventRecord(e1, st);
+        if (cudaEventSynchronize(e1) != cudaSuccess) break;
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (ms > 0.f) best_bw = std::max(best_bw, (float)((double)n4 * 16 * sweeps / (ms * 1e-3) / 1e9));
+    }
+    const int iters = 20000;
+    for (int r = 0; r < reps; ++r) {
+        cudaEventRecord(e0, st);
+        k_fma_rate<<<sms * 8, 256, 0, st>>>(iters, sink);
+        cudaEventRecord(e1, st);
+        if (cudaEventSynchronize(e1) != cudaSuccess) break;
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (ms > 0.f) best_fl = std::max(best_fl, (float)((double)sms * 8 * 256 * iters * 8 * 2 / (ms * 1e-3) / 1e12));
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaError_t e = cudaGetLastError();
+    cudaFree(buf); cudaFree(sink);
+    if (e != cudaSuccess) { set_error(std::string("tomo_measure_device: ") + cudaGetErrorString(e)); return TOMO_ECUDA; }
+    out[0] = best_bw; out[1] = best_fl;
+    return TOMO_OK;
+}
+
 extern "C" int tomo_get_sizes(const tomo_plan *pl, int *n_vs, int *n_vphi, int *slopes_len, int *wavefront_len,
                               int *pad, int *pad_os, int *n_prime) {
     if (!pl) { set_error("plan is NULL"); return TOMO_EINVAL; }

@@ -23,7 +23,7 @@ TOMO_SOLVER_MULTIKERNEL, TOMO_SOLVER_PERSISTENT = 0, 1
 
 EXPORTS = (
     "tomo_plan_create", "tomo_plan_upload_kernels", "tomo_solve", "tomo_solve_batch", "tomo_solve_minres", "tomo_apply_css",
-    "tomo_apply_cos", "tomo_cg_step", "tomo_get_zeta", "tomo_time_kernels", "tomo_time_phases", "tomo_time_solver",
+    "tomo_apply_cos", "tomo_cg_step", "tomo_get_zeta", "tomo_time_kernels", "tomo_time_phases", "tomo_time_solver", "tomo_measure_device",
     "tomo_get_sizes", "tomo_get_valid_index", "tomo_get_noise",
     "tomo_get_residuals", "tomo_get_stats", "tomo_plan_destroy", "tomo_last_error",
     "tomo_host_sizes", "tomo_host_css_generators", "tomo_host_cos_generators", "tomo_host_generator_spectrum",
@@ -105,6 +105,7 @@ def load(build_if_missing: bool = True):
                                              C.c_int, dp]
     lib.tomo_host_generator_spectrum.argtypes = [dp, C.c_int, C.c_int, C.c_int, dp]
     lib.tomo_host_structure_function.argtypes = [dp, C.c_int, C.c_double, C.c_double, dp]
+    lib.tomo_measure_device.argtypes = [C.c_longlong, C.c_int, C.POINTER(C.c_float), vp]
     lib.tomo_host_slab_segments.argtypes = [C.c_int, C.c_int, C.c_int, ip]
     _lib = lib
     return lib
@@ -180,6 +181,14 @@ def host_structure_function(r, r0: float, L0: float) -> np.ndarray:
     out = np.empty_like(rr)
     _check(lib.tomo_host_structure_function(_dp(rr), rr.size, r0, L0, _dp(out)))
     return out.reshape(np.shape(r))
+
+
+def measure_device(l2_bytes: int = 0, reps: int = 5, stream=None):
+    """L2 -> SM read bandwidth [GB/s] and plain fp32 FMA rate [TFLOP/s] of the current device (tomo_measure_device)."""
+    lib = load()
+    out = (C.c_float * 2)()
+    _check(lib.tomo_measure_device(l2_bytes, reps, out, _stream_handle(stream)))
+    return {"l2_read_GBps": float(out[0]), "fp32_TFLOPs": float(out[1])}
 
 
 def host_slab_segments(Ph: int, n_frames: int, n_ctas: int) -> np.ndarray:
