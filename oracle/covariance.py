@@ -12,6 +12,9 @@ stencil {(o_m, w_m)} with sum w = 0,
 (Eq.49 L598 and the identity at L600); Eq.50-52 and Eq.56-62 are special cases and are
 checked against this function in tests/test_oracle_covariance.py.
 
+A third model, the FFT slope model (Eq.41-46: the gradient averaged over the subaperture), is not a stencil; it
+lives in fftmodel.py and is reached through the same two functions with model="fft".
+
 Layers (L562, reading G8): D_phi,k = f_k D_phi, covariances add over layers.
 Cone effect (L158, reading G7): at layer k a subaperture of an LGS WFS j sits at
 gamma_k r_q + h_k alpha_j, its stencil arms are d_k = gamma_k d long, the
@@ -51,6 +54,9 @@ def cov_slope_slope(delta, a: int, b: int, width: float, c: float, r0: float, L0
 
     delta: (..., 2) separation [m] (second minus first); width: local subaperture size d_k;
     c: slope normalisation (1/d)."""
+    if model == "fft":           # subaperture-averaged gradient, Eq.41-45 (not a stencil)
+        from . import fftmodel
+        return fftmodel.cov_slope_slope(delta, a, b, width, c, r0, L0)
     delta = np.asarray(delta, dtype=np.float64)
     out = np.zeros(delta.shape[:-1])
     for (off, w) in _merged_pairs(STENCILS[model][a], STENCILS[model][b]):
@@ -63,6 +69,9 @@ def cov_slope_slope(delta, a: int, b: int, width: float, c: float, r0: float, L0
 def cov_phase_slope(delta, b: int, width: float, c: float, r0: float, L0: float,
                     model: str = "hudgin"):
     """cov(phi(r_p), s_b(r_p + delta)) for one layer of unit Cn2 fraction (delta = r_q - r_p)."""
+    if model == "fft":           # Eq.46
+        from . import fftmodel
+        return fftmodel.cov_phase_slope(delta, b, width, c, r0, L0)
     delta = np.asarray(delta, dtype=np.float64)
     out = np.zeros(delta.shape[:-1])
     for (off, w) in STENCILS[model][b]:
