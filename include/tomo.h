@@ -37,6 +37,9 @@ extern "C" {
 
 #define TOMO_HUDGIN 0          /* Eq.47-52 (L584-615), default slope model                                            */
 #define TOMO_FRIED  1          /* Eq.54-62 (L630-691)                                                                 */
+#define TOMO_FFTMODEL 2        /* Eq.41-46 (L534-572): gradient averaged over the subaperture; the covariances are    */
+                               /* Fourier integrals of the von Karman spectrum, evaluated by the builder with 2-D FFTs */
+                               /* on a grid of edge >= 512 and pixel d_k/4 (reading G29 of DESIGN.md)                  */
 
 #define TOMO_F32       0       /* fp32 storage and arithmetic (headline path)                                         */
 #define TOMO_F32S_F64A 1       /* fp32-stored spectra, fp64 FFT / vectors                                             */
@@ -86,7 +89,7 @@ typedef struct {
 } tomo_noise;
 
 typedef struct {
-    int slope_model;                   /* TOMO_HUDGIN | TOMO_FRIED                                                   */
+    int slope_model;                   /* TOMO_HUDGIN | TOMO_FRIED | TOMO_FFTMODEL                                   */
     int pad;                           /* FFT edge P for Sigma_ss, 0 = next even 2^a 3^b 5^c >= 2n-1   (L207, G11)    */
     int pad_os;                        /* FFT edge P_os for Sigma_phi-s, 0 = next even 5-smooth >= n'+n-1            */
     int max_batch;                     /* largest n_frames a solve may be given (>= 1)                               */

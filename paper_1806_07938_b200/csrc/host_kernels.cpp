@@ -51,12 +51,73 @@ struct Lattice {
         return v;
     }
 };
+
+// ---- FFT slope model (Eq.41-46; reading G29).  The slope is the gradient averaged over the subaperture; with
+// H(f) = sinc(w f_x) sinc(w f_y) (Eq.44), the von Karman spectrum Phi (Eq.45, constant 0.0229: G3), slopes in rad/m and
+// the cone compression gamma = w/d (L158):
+//   cov(s_a(r), s_b(r + D))     = gamma^2 int (2 pi)^2 f_a f_b Phi H^2 cos(2 pi f.D) d^2f      (Eq.43)
+//   cov(phi(r_p), s_b(r_p + D)) = -gamma  int  2 pi f_b      Phi H   sin(2 pi f.D) d^2f        (Eq.46)
+// "computed by the FFT, accuracy depends on the sampling" (L572): Riemann sum over the grid of an FFT of edge NG with pixel
+// w / kFftOver: f = p df, |p| < NG/2 (the unpaired Nyquist sample is left out), df = kFftOver / (NG w).  One inverse 2-D FFT
+// gives the sum at every separation q (w / kFftOver) + shift; the lags of a generator are every kFftOver-th sample.
+const int kFftOver = 4;
+// Eq.45's constant, exact: (24 Gamma(6/5)/5)^(5/6) Gamma(11/6)^2 / (2 pi^(11/3)) = 0.022896 (the paper prints 0.029: G3)
+const double kPsdConst = std::pow(24.0 * std::tgamma(6.0 / 5.0) / 5.0, 5.0 / 6.0) * std::tgamma(11.0 / 6.0) * std::tgamma(11.0 / 6.0) /
+                         (2.0 * std::pow(M_PI, 11.0 / 3.0));
+
+int fft_grid_edge(int max_lag) {                      // power of two, >= 512, lags up to max_lag representable
+    int ng = 512;
+    while (kFftOver * max_lag >= ng / 2) ng *= 2;
+    return ng;
+}
+double sinc_pi(double x) { return x == 0.0 ? 1.0 : std::sin(M_PI * x) / (M_PI * x); }
+
+// tab[(qy mod NG) NG + (qx mod NG)] = sum_p weight(fx, fy) exp(2 pi i f.(q w/kFftOver + shift)); kind 0/1/2 = Sigma_ss xx / yy / xy
+// (real part), 3/4 = Sigma_phi-s x / y (imaginary part)
+void fft_model_table(int NG, double w, double gam, double r0, double L0, double shx, double shy, int kind,
+                     std::vector<std::complex<double>> &tab) {
+    typedef std::complex<double> cd;
+    const double df = kFftOver / (NG * w);
+    tab.assign((size_t)NG * NG, cd(0, 0));
+    for (int py = -(NG / 2 - 1); py < NG / 2; ++py)
+        for (int px = -(NG / 2 - 1); px < NG / 2; ++px) {
+            const double fx = px * df, fy = py * df;
+            const double H = sinc_pi(w * fx) * sinc_pi(w * fy);
+            const double phi = kPsdConst * std::pow(r0, -5.0 / 3.0) * std::pow(fx * fx + fy * fy + 1.0 / (L0 * L0), -11.0 / 6.0);
+            double wt;
+            if (kind < 3) {
+                const double fa = (kind == 1) ? fy : fx, fb = (kind == 0) ? fx : fy;
+                wt = gam * gam * 4.0 * M_PI * M_PI * fa * fb * phi * H * H * df * df;
+            } else {
+                wt = -gam * 2.0 * M_PI * (kind == 3 ? fx : fy) * phi * H * df * df;
+            }
+            const double ph = 2.0 * M_PI * (fx * shx + fy * shy);
+            tab[(size_t)((py + NG) % NG) * NG + ((px + NG) % NG)] = wt * cd(std::cos(ph), std::sin(ph));
+        }
+    for (int y = 0; y < NG; ++y) host_fft(&tab[(size_t)y * NG], NG, 1, true);       // inverse: exp(+2 pi i p q / NG), unscaled
+    for (int x = 0; x < NG; ++x) host_fft(&tab[x], NG, NG, true);
+}
 }  // namespace
 
 // 1/2 [theta_x0x0(0) + theta_y0y0(0)]: the model slope variance the noise level is quoted against (reading G15)
 double model_slope_variance(const HostModel &m) {
     double v = 0.0;
     const double c = 1.0 / m.d;
+    if (m.slope_model == TOMO_FFTMODEL) {
+        const int NG = fft_grid_edge(m.n_p);
+        for (int k = 0; k < m.K; ++k) {
+            const double w = m.gamma[k] * m.d, df = kFftOver / (NG * w);
+            double s = 0.0;
+            for (int py = -(NG / 2 - 1); py < NG / 2; ++py)
+                for (int px = -(NG / 2 - 1); px < NG / 2; ++px) {
+                    const double fx = px * df, fy = py * df, H = sinc_pi(w * fx) * sinc_pi(w * fy);
+                    const double phi = kPsdConst * std::pow(m.r0, -5.0 / 3.0) * std::pow(fx * fx + fy * fy + 1.0 / (m.L0 * m.L0), -11.0 / 6.0);
+                    s += 4.0 * M_PI * M_PI * (fx * fx + fy * fy) * phi * H * H * df * df;
+                }
+            v += m.frac[k] * m.gamma[k] * m.gamma[k] * s;
+        }
+        return 0.5 * v;
+    }
     for (int k = 0; k < m.K; ++k) {
         const double w = m.gamma[k] * m.d;
         Lattice lat(-2, 2, 0.5 * w, 0.0, 0.0, m.r0, m.L0);
@@ -93,6 +154,21 @@ void build_css_generators(const HostModel &m, std::vector<double> &gen) {
         for (int k = 0; k < K; ++k) {
             const double w = m.gamma[k] * m.d;
             const double shx = m.h[k] * (m.ax[j] - m.ax[i]), shy = m.h[k] * (m.ay[j] - m.ay[i]);
+            if (m.slope_model == TOMO_FFTMODEL) {
+                const int NG = fft_grid_edge(m.n_p);
+                std::vector<std::complex<double>> tab;
+                for (int a = 0; a < 2; ++a)
+                    for (int b = a; b < 2; ++b) {
+                        fft_model_table(NG, w, m.gamma[k], m.r0, m.L0, shx, shy, a == b ? a : 2, tab);
+                        for (int ly = -(n - 1); ly < n; ++ly)
+                            for (int lx = -(n - 1); lx < n; ++lx) {
+                                const double val = m.frac[k] * tab[(size_t)((kFftOver * ly + NG) % NG) * NG + ((kFftOver * lx + NG) % NG)].real();
+                                tmp[((size_t)k * 4 + a * 2 + b) * LL + (size_t)(ly + n - 1) * L + (lx + n - 1)] = val;
+                                if (a != b) tmp[((size_t)k * 4 + b * 2 + a) * LL + (size_t)(ly + n - 1) * L + (lx + n - 1)] = val;
+                            }
+                    }
+                continue;
+            }
             Lattice lat(-2 * n, 2 * n, 0.5 * w, shx, shy, m.r0, m.L0);
             const double scale = m.frac[k] * (-0.5 * c * c);
             for (int a = 0; a < 2; ++a)
@@ -150,6 +226,19 @@ void build_cos_generators(const HostModel &m, int target, std::vector<double> &g
             const double off = w * ((np - 1) / 2.0 - (n - 1) / 2.0);
             const double shx = off + m.h[k] * (m.ax[j] - m.bx[target]);
             const double shy = off + m.h[k] * (m.ay[j] - m.by[target]);
+            if (m.slope_model == TOMO_FFTMODEL) {
+                const int NG = fft_grid_edge(m.n_p);
+                std::vector<std::complex<double>> tab;
+                for (int b = 0; b < 2; ++b) {
+                    fft_model_table(NG, w, m.gamma[k], m.r0, m.L0, shx, shy, 3 + b, tab);
+                    double *o = m.lgs ? &gen[((size_t)k * C + 2 * j + b) * LL] : &tmp[((size_t)k * C + 2 * j + b) * LL];
+                    for (int ly = -(np - 1); ly < n; ++ly)
+                        for (int lx = -(np - 1); lx < n; ++lx)
+                            o[(size_t)(ly + np - 1) * Los + (lx + np - 1)] =
+                                m.frac[k] * tab[(size_t)((kFftOver * ly + NG) % NG) * NG + ((kFftOver * lx + NG) % NG)].imag();
+                }
+                continue;
+            }
             Lattice lat(-2 * np, 2 * n, 0.5 * w, shx, shy, m.r0, m.L0);
             const double scale = m.frac[k] * (-0.5 * c);
             for (int b = 0; b < 2; ++b) {

@@ -83,7 +83,7 @@ int build_model(const tomo_geometry *g, const tomo_cn2 *cn2, double r0, double L
     if (!(r0 > 0) || !(L0 > 0)) { err = "r0 and L0 must be positive"; return TOMO_EINVAL; }
     if (g->n_targets < 0 || (g->n_targets > 0 && !g->target_xy)) { err = "bad targets"; return TOMO_EINVAL; }
     if (g->n_lo < 0 || (g->n_lo > 0 && !g->lo_wfs)) { err = "bad low-order sensor list"; return TOMO_EINVAL; }
-    if (slope_model != TOMO_HUDGIN && slope_model != TOMO_FRIED) { err = "unknown slope model"; return TOMO_EINVAL; }
+    if (slope_model != TOMO_HUDGIN && slope_model != TOMO_FRIED && slope_model != TOMO_FFTMODEL) { err = "unknown slope model"; return TOMO_EINVAL; }
     if (g->obstruction < 0 || g->obstruction >= 1) { err = "obstruction must be in [0,1)"; return TOMO_EINVAL; }
     m = HostModel();
     m.n = g->n; m.D = g->D; m.d = g->D / g->n; m.r0 = r0; m.L0 = L0; m.obstruction = g->obstruction;

@@ -17,7 +17,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libtomo_b200.so")
 
 TOMO_OK, TOMO_EINVAL, TOMO_EUNSUPPORTED, TOMO_ENOTREADY, TOMO_ENOMEM, TOMO_ECUDA = 0, -1, -2, -3, -4, -5
-TOMO_HUDGIN, TOMO_FRIED = 0, 1
+TOMO_HUDGIN, TOMO_FRIED, TOMO_FFTMODEL = 0, 1, 2
 TOMO_F32, TOMO_F32S_F64A, TOMO_F64 = 0, 1, 2
 TOMO_SOLVER_MULTIKERNEL, TOMO_SOLVER_PERSISTENT = 0, 1
 

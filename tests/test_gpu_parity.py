@@ -55,6 +55,8 @@ def _case(name):
         return replace(c, obstruction=0.3), "hudgin", None
     if name == "small_fried":
         return small_lgs_config(n=8, n_gs=2, n_layers=2, targets=((2.0, 1.0),)), "fried", None
+    if name == "small_fftmodel":     # FFT slope model (Eq.41-46): covariances by 2-D FFTs in the builder
+        return small_lgs_config(n=8, n_gs=3, n_layers=2, targets=((3.0, -2.0),)), "fft", None
     if name == "ngs_offaxis":        # NGS, one WFS with tip/tilt removed and one without, off-axis target
         c = get_config("cfg1")
         return replace(c, wfs=(WFS(10.0, 0.0, float("inf"), 2), WFS(-10.0, 5.0)), targets=((3.0, 4.0),)), "hudgin", None
@@ -75,7 +77,7 @@ def system(name):
 
 def make_plan(name, **kw):
     cfg, model, osys, _ = system(name)
-    sm = tomo.TOMO_FRIED if model == "fried" else tomo.TOMO_HUDGIN
+    sm = {"fried": tomo.TOMO_FRIED, "fft": tomo.TOMO_FFTMODEL}.get(model, tomo.TOMO_HUDGIN)
     pl = tomo.TomoPlan(cfg, slope_model=sm, **kw)
     s2, var = pl.noise()
     assert abs(s2[0] / osys.sigma2 - 1) < 1e-12 and abs(var / osys.slope_var - 1) < 1e-12
@@ -84,7 +86,7 @@ def make_plan(name, **kw):
     return pl
 
 
-ALL = ["cfg1", "small_lgs", "small_odd_focus", "small_fried", "ngs_offaxis", "cfg2"]
+ALL = ["cfg1", "small_lgs", "small_odd_focus", "small_fried", "small_fftmodel", "ngs_offaxis", "cfg2"]
 # both solvers go through every solve gate: the multi-kernel CUDA-graph loop and the persistent cooperative kernel
 SOLVERS = [tomo.TOMO_SOLVER_MULTIKERNEL, tomo.TOMO_SOLVER_PERSISTENT]
 solvers = pytest.mark.parametrize("solver", SOLVERS, ids=["multikernel", "persistent"])
@@ -182,7 +184,7 @@ def test_free_running_fp32_tracks_oracle_up_to_the_fp32_horizon(name, solver):
 
 # ------------------------------------------------------------------------------------------------ P-d
 @solvers
-@pytest.mark.parametrize("name", ["cfg1", "small_lgs", "small_odd_focus", "small_fried", "ngs_offaxis", "cfg2"])
+@pytest.mark.parametrize("name", ["cfg1", "small_lgs", "small_odd_focus", "small_fried", "small_fftmodel", "ngs_offaxis", "cfg2"])
 def test_converged_solution_matches_direct_solve(name, solver):
     cfg, _, osys, data = system(name)
     s = f32(data["slopes"][0].ravel())

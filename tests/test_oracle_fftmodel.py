@@ -77,3 +77,21 @@ def test_model_variance_is_below_hudgin_and_dispatch_through_covariance():
     v_hud = cov.cov_slope_slope(z, 0, 0, W, 1 / W, R0, L0, "hudgin")[0]
     assert 0.5 * v_hud < v_fft < v_hud
     assert v_fft == fm.cov_slope_slope(z, 0, 0, W, 1 / W, R0, L0)[0]
+
+
+def test_end_to_end_with_the_fft_model_reduces_error_and_pins_signs():
+    """MMSE reconstruction with the FFT-model covariances on screen-generated (two-point) slopes: the estimate must follow the
+    true phase -- this fixes the sign of Eq.46 and the gamma / 2 pi factors at once (a flipped sign gives an error > 1)."""
+    from oracle.system import OracleSystem
+    from tomo_inputs import get_config, screens
+    from tomo_inputs.configs import small_lgs_config
+    for cfg in (get_config("cfg1"), small_lgs_config(n=8, n_gs=3, n_layers=2)):
+        s = OracleSystem(cfg, model="fft")
+        inp = screens.generate(cfg, s.sigma2)
+        phi = s.reconstruct(s.solve_direct(inp["slopes"][0].ravel()))
+        truth = s.Mphi @ inp["truth"][0, 0]
+        assert np.linalg.norm(phi - truth) / np.linalg.norm(truth) < 0.7
+        assert np.corrcoef(phi, truth)[0, 1] > 0.75
+        assert np.linalg.norm(-phi - truth) / np.linalg.norm(truth) > 1.2
+        w = np.linalg.eigvalsh(s.Css)
+        assert w.min() > -1e-9 * w.max()                                  # a covariance matrix
