@@ -633,9 +633,42 @@ template <typename T, typename S> struct Ops {
         return rc;
     }
 
+    // A7-A8 after the persistent solver: the seven small kernels are replayed from one CUDA graph per frame count (their
+    // arguments are plan-owned buffers), which shortens the gaps between the dependent launches
     static int project_from_x(tomo_plan *pl, cudaStream_t st, int F) {
         int rc;
         if ((rc = prepare(pl))) return rc;
+        const char *no_graph = getenv("TOMO_NO_GRAPH");
+        if (!(no_graph && no_graph[0] == '1')) {
+            const auto key = std::make_tuple(F, -1, 8);
+            auto it = pl->graphs.find(key);
+            if (it == pl->graphs.end()) {
+                const int before = pl->launches_last;
+                cudaStream_t cs;
+                CK(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
+                CK(cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal));
+                rc = project_from_x_enqueue(pl, cs, F);
+                cudaGraph_t graph = nullptr;
+                cudaError_t e = cudaStreamEndCapture(cs, &graph);
+                cudaStreamDestroy(cs);
+                if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+                if (e != cudaSuccess) { set_error(std::string("graph capture: ") + cudaGetErrorString(e)); return TOMO_ECUDA; }
+                cudaGraphExec_t exec = nullptr;
+                e = cudaGraphInstantiate(&exec, graph, 0);
+                cudaGraphDestroy(graph);
+                if (e != cudaSuccess) { set_error(std::string("graph instantiate: ") + cudaGetErrorString(e)); return TOMO_ECUDA; }
+                it = pl->graphs.emplace(key, exec).first;
+                pl->graph_launches[key] = pl->launches_last - before;
+            } else {
+                pl->launches_last += pl->graph_launches[key];
+            }
+            CK(cudaGraphLaunch(it->second, st));
+            return TOMO_OK;
+        }
+        return project_from_x_enqueue(pl, st, F);
+    }
+
+    static int project_from_x_enqueue(tomo_plan *pl, cudaStream_t st, int F) {
         ProjectArgs<T, T> pa;
         pa.g = pl->g; pa.in = (const T *)pl->d_x; pa.out = (T *)pl->d_z; pa.out2 = pa.out3 = pa.zero = nullptr;
         pa.partials_r = nullptr; pa.part_stride = 0;
