@@ -287,8 +287,10 @@ def main():
         kb = n_iter * b_iter + B * 4 * Ns * E
         ach = kb / (k_ms * 1e-3) / 1e9
         roof = {"kernel": "k_persistent", "bound": "hbm", "achieved": ach, "peak": hbm, "unit": "GB/s", "frac": ach / hbm,
-                # dram__bytes_read.sum + dram__bytes_write.sum of one launch, ncu --set full (profiles/r1_persistent_ncu_details.md)
-                "traffic": 8674048 if (cfg.name.startswith("cfg3") and B == 1 and args.precision == "f32") else None,
+                # dram__bytes_read.sum + dram__bytes_write.sum of one launch, ncu --set full (profiles/r1_persistent_ncu_details.md:
+                # 8.550 MB + 0.133 MB at batch 1, 11.71 MB + 36.45 MB at batch 16)
+                "traffic": 8683264 if (cfg.name.startswith("cfg3") and B == 1 and args.precision == "f32") else
+                           (48158976 if (cfg.name.startswith("cfg3") and B == 16 and args.precision == "f32") else None),
                 "peak_source": how, "algorithmic_bytes_per_launch": kb,
                 "ms_per_launch": k_ms, "ms_per_launch_n_iter0": k_ms0,
                 "us_per_iteration_in_kernel": (k_ms - k_ms0) / n_iter * 1e3,
