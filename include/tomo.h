@@ -196,6 +196,20 @@ int tomo_get_residuals(const tomo_plan *plan, double *host_out, int n_frames, in
 /* Bytes of device memory owned by the plan, and the number of kernel launches the last solve enqueued. */
 int tomo_get_stats(const tomo_plan *plan, long long *device_bytes, int *launches_last_solve);
 
+/* ---- split low-order path for the NGS tip/tilt sensors of geom->lo_wfs (L321, L412, Table 2; the paper gives no
+ * algorithm: reading G30 of DESIGN.md).  Each low-order sensor delivers the mean x- and the mean y-slope over the valid
+ * subapertures [rad/m] with white noise of variance sigma2_lo; R_lo = C_tau,g (C_gg + sigma2_lo I)^-1 (Eq.5 L68 on the
+ * aperture-mean slope pairs, [2 n_targets][2 n_lo]) is built once on the host (stencil slope models only: EUNSUPPORTED for
+ * TOMO_FFTMODEL; EINVAL when n_lo == 0 or the matrix is not positive definite) and uploaded.  *out owns its device memory. */
+typedef struct tomo_lo tomo_lo;
+int tomo_lo_create(const tomo_geometry *geom, const tomo_cn2 *cn2, double r0, double L0, int slope_model, double sigma2_lo,
+                   tomo_lo **out);
+/* wavefront[frame][target][valid phase point] += tau_x x_p + tau_y y_p, tau = R_lo g_frame, in place on `cuda_stream`
+ * (asynchronous).  lo_slopes: DEVICE fp32 [n_frames][n_lo][2 (x, y)]; wavefront: DEVICE fp32 in the layout tomo_solve_batch
+ * writes (the tip/tilt-free high-order estimate, Eq.35).  n_frames in [0, 65535]; 0 = no launch (buffers may be NULL). */
+int tomo_lo_apply(const tomo_lo *lo, const float *lo_slopes, float *wavefront, int n_frames, void *cuda_stream);
+void tomo_lo_destroy(tomo_lo *lo);
+
 void tomo_plan_destroy(tomo_plan *plan);
 const char *tomo_last_error(void);
 

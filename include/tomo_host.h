@@ -32,6 +32,12 @@ int tomo_host_generator_spectrum(const double *gen, int n_out, int n_in, int P, 
 /* D_phi(r) of Eq.53 (L619) for count separations r [m]. */
 int tomo_host_structure_function(const double *r, int count, double r0, double L0, double *out);
 
+/* Low-order NGS tip/tilt estimator of tomo_lo_create (reading G30; L321, L412) without a device.  M = n_lo + n_targets
+ * directions, sensors first.  R_out: host [2 n_targets][2 n_lo] row-major, order [direction][x, y]; cov_out: host [2M][2M]
+ * covariance of the aperture-mean slope pairs (without the noise term).  Either may be NULL. */
+int tomo_host_lo_estimator(const tomo_geometry *geom, const tomo_cn2 *cn2, double r0, double L0, int slope_model,
+                           double sigma2_lo, double *R_out, double *cov_out);
+
 /* Work table of the persistent solver's batch path: how the Ph x n_frames slab passes of one CG iteration (one k_x slab of
  * all channels of one frame: y-FFTs + the per-frequency block product, Eq.22 / Eq.30) are dealt to n_ctas CTAs.  CTA b
  * owns slab b % Ph with the other CTAs of that residue; CTAs above the average hand frames to CTAs below it (one helped

@@ -17,13 +17,16 @@ What it computes (each module cites the passage it follows, PAPER.md L<line>):
   toeplitz.py    the paper's 2RBT product Eq.18-28 step by step, generators, op counts
   directsum.py   matrix-free direct-sum MVM for ELT sizes (directsum.c, OpenMP)
   system.py      assembles a TomoConfig into the operator A, rhs and projections
+  loworder.py    low-order NGS tip/tilt path (paper-silent, L321/L412; reading G30): MMSE estimator of the aperture-mean
+                 slopes from positions, tilt add-back
 
 Pins (tests/test_oracle_*.py, `-m "not gpu"`): closed forms of D_phi, the Kolmogorov
 limit, the PSD integral, printed formulas Eq.50-52 / Eq.56-62 against the generic
 stencil evaluation, symmetry/PSD of C_ss, dense == paper's index maps == 2-D FFT
 product, projector identities, CG -> Cholesky, MINRES = the least-squares minimiser over the
 Krylov space (brute force) = scipy's minres, LGS ground-layer identity, the
-paper's printed closed-form counts (L150, L177, L197, L270, L280, L295).
+paper's printed closed-form counts (L150, L177, L197, L270, L280, L295), the telescoping
+closed form of the aperture-mean Hudgin slope variance (loworder.py).
 
 Parity unpinned: absolute WFE in nm (Table 3) and the curves of Fig.9-15 are not
 reproduced; nothing in this package depends on them.

@@ -17,7 +17,7 @@ LIB = os.path.join(HERE, "libtomo_b200.so")
 OBJ = os.path.join(HERE, "build")
 
 PERSIST_SIZES = [16, 20, 24, 32, 40, 64, 128, 160, 192, 256]     # TOMO_PERSIST_SIZES in csrc/persist_host.cuh
-CU = [("tomo_api.cu", "tomo_api", []), ("solve_persistent.cu", "solve_persistent", [])] + \
+CU = [("tomo_api.cu", "tomo_api", []), ("solve_persistent.cu", "solve_persistent", []), ("lo_path.cu", "lo_path", [])] + \
      [("persist_inst.cu", f"persist_inst_{p}", [f"-DTOMO_PINST={p}"]) for p in PERSIST_SIZES]
 CPP = ["host_model.cpp", "host_kernels.cpp"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -207,6 +207,84 @@ void build_css_generators(const HostModel &m, std::vector<double> &gen) {
     }
 }
 
+// ------------------------------------------------------------------------------------------------ low-order NGS path
+// Reading G30 (the paper is silent: L321, L412).  Sensor m and target t are described by the aperture-mean slope pair in
+// their direction (NGS / infinity: no cone compression).  With c(l) the autocorrelation count of the subaperture mask,
+//   cov(mean_a(u), mean_b(v)) = 1/n_vs^2 sum_l c(l) sum_k f_k cov_ab(d l + h_k (v - u); d)
+// (the same cov_ab as Sigma_ss, Eq.49).  R_lo = C_tau,g (C_gg + sigma2_lo I)^-1 by Cholesky (Eq.5).
+int build_lo_estimator(const HostModel &m, const std::vector<double> &ux, const std::vector<double> &uy, int n_lo,
+                       double sigma2_lo, std::vector<double> &R, std::vector<double> &Cm) {
+    const int n = m.n, L = 2 * n - 1, K = m.K, M = (int)ux.size(), T = M - n_lo, n_g = 2 * n_lo;
+    const size_t LL = (size_t)L * L;
+    std::vector<double> cnt(LL, 0.0);
+    for (int q = 0; q < m.nv; ++q)
+        for (int p = 0; p < m.nv; ++p) cnt[(size_t)(m.iy[p] - m.iy[q] + n - 1) * L + (m.ix[p] - m.ix[q] + n - 1)] += 1.0;
+    std::vector<Tap> st[2][2];
+    for (int a = 0; a < 2; ++a)
+        for (int b = 0; b < 2; ++b) st[a][b] = pair_stencil(m.slope_model, a, b);
+    const double c = 1.0 / m.d, inv = 1.0 / ((double)m.nv * m.nv);
+    Cm.assign((size_t)4 * M * M, 0.0);
+    std::vector<std::pair<int, int>> pairs;
+    for (int i = 0; i < M; ++i)
+        for (int j = i; j < M; ++j) pairs.push_back({i, j});
+#pragma omp parallel for schedule(dynamic)
+    for (int e = 0; e < (int)pairs.size(); ++e) {
+        const int i = pairs[e].first, j = pairs[e].second;
+        double acc[2][2] = {{0, 0}, {0, 0}};
+        for (int k = 0; k < K; ++k) {
+            Lattice lat(-2 * n, 2 * n, 0.5 * m.d, m.h[k] * (ux[j] - ux[i]), m.h[k] * (uy[j] - uy[i]), m.r0, m.L0);
+            for (int a = 0; a < 2; ++a)
+                for (int b = 0; b < 2; ++b) {
+                    double s = 0.0;
+                    for (int ly = -(n - 1); ly < n; ++ly)
+                        for (int lx = -(n - 1); lx < n; ++lx) {
+                            const double w = cnt[(size_t)(ly + n - 1) * L + (lx + n - 1)];
+                            if (w == 0.0) continue;
+                            double v = 0.0;
+                            for (const Tap &t : st[a][b]) v += t.w * lat.get(2 * lx + t.u, 2 * ly + t.v);
+                            s += w * v;
+                        }
+                    acc[a][b] += m.frac[k] * (-0.5 * c * c) * s * inv;
+                }
+        }
+        for (int a = 0; a < 2; ++a)
+            for (int b = 0; b < 2; ++b) {
+                Cm[(size_t)(2 * i + a) * 2 * M + (2 * j + b)] = acc[a][b];
+                Cm[(size_t)(2 * j + b) * 2 * M + (2 * i + a)] = acc[a][b];
+            }
+    }
+    // Cholesky of A = C_gg + sigma2_lo I, then R^T = A^-1 C_g,tau column by column
+    std::vector<double> A((size_t)n_g * n_g);
+    for (int r = 0; r < n_g; ++r)
+        for (int q = 0; q < n_g; ++q) A[(size_t)r * n_g + q] = Cm[(size_t)r * 2 * M + q] + (r == q ? sigma2_lo : 0.0);
+    for (int r = 0; r < n_g; ++r)
+        for (int q = 0; q <= r; ++q) {
+            double s = A[(size_t)r * n_g + q];
+            for (int p = 0; p < q; ++p) s -= A[(size_t)r * n_g + p] * A[(size_t)q * n_g + p];
+            if (r == q) {
+                if (!(s > 0.0)) return TOMO_EINVAL;
+                A[(size_t)r * n_g + r] = std::sqrt(s);
+            } else {
+                A[(size_t)r * n_g + q] = s / A[(size_t)q * n_g + q];
+            }
+        }
+    R.assign((size_t)2 * T * n_g, 0.0);
+    std::vector<double> y(n_g);
+    for (int row = 0; row < 2 * T; ++row) {
+        for (int r = 0; r < n_g; ++r) {
+            double s = Cm[(size_t)(n_g + row) * 2 * M + r];
+            for (int p = 0; p < r; ++p) s -= A[(size_t)r * n_g + p] * y[p];
+            y[r] = s / A[(size_t)r * n_g + r];
+        }
+        for (int r = n_g - 1; r >= 0; --r) {
+            double s = y[r];
+            for (int p = r + 1; p < n_g; ++p) s -= A[(size_t)p * n_g + r] * R[(size_t)row * n_g + p];
+            R[(size_t)row * n_g + r] = s / A[(size_t)r * n_g + r];
+        }
+    }
+    return TOMO_OK;
+}
+
 // ------------------------------------------------------------------------------------------------ Sigma_phi-s
 // xi'[k,(j,b)](l) = f_k cov_phi,b(d_k l + d_k[(n'-1)/2 - (n-1)/2] + h_k (alpha_j - beta); d_k),  l = q - p'
 // cov_phi,b(Delta; w) = -1/2 c sum_m' w'_m' D_phi(|Delta + o'_m'|)            (Eq.52; L179-197; reading G18)

@@ -62,6 +62,12 @@ void build_css_generators(const HostModel &m, std::vector<double> &gen);
 // xi'[k,(j,b)](l) for one target: gen[Kp][C][Los][Los], Los = n'+n-1.
 void build_cos_generators(const HostModel &m, int target, std::vector<double> &gen);
 
+// Low-order NGS tip/tilt estimator (reading G30; L321, L412): directions (ux, uy) [rad] = n_lo sensors then the T targets.
+// Cm: covariance of the aperture-mean slope pairs [2M][2M]; R = C_tau,g (C_gg + sigma2_lo I)^-1, [2T][2 n_lo] row-major.
+// Returns TOMO_EINVAL when C_gg + sigma2_lo I is not positive definite.
+int build_lo_estimator(const HostModel &m, const std::vector<double> &ux, const std::vector<double> &uy, int n_lo,
+                       double sigma2_lo, std::vector<double> &R, std::vector<double> &Cm);
+
 // 1/2 [theta_x0x0(0) + theta_y0y0(0)] without building the whole table.
 double model_slope_variance(const HostModel &m);
 

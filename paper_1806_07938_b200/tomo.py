@@ -28,6 +28,7 @@ EXPORTS = (
     "tomo_get_residuals", "tomo_get_stats", "tomo_plan_destroy", "tomo_last_error",
     "tomo_host_sizes", "tomo_host_css_generators", "tomo_host_cos_generators", "tomo_host_generator_spectrum",
     "tomo_host_structure_function", "tomo_host_slab_segments",
+    "tomo_host_lo_estimator", "tomo_lo_create", "tomo_lo_apply", "tomo_lo_destroy",
 )
 
 
@@ -107,6 +108,13 @@ def load(build_if_missing: bool = True):
     lib.tomo_host_structure_function.argtypes = [dp, C.c_int, C.c_double, C.c_double, dp]
     lib.tomo_measure_device.argtypes = [C.c_longlong, C.c_int, C.POINTER(C.c_float), vp]
     lib.tomo_host_slab_segments.argtypes = [C.c_int, C.c_int, C.c_int, ip]
+    lib.tomo_host_lo_estimator.argtypes = [C.POINTER(_Geometry), C.POINTER(_Cn2), C.c_double, C.c_double, C.c_int,
+                                           C.c_double, dp, dp]
+    lib.tomo_lo_create.argtypes = [C.POINTER(_Geometry), C.POINTER(_Cn2), C.c_double, C.c_double, C.c_int, C.c_double,
+                                   C.POINTER(vp)]
+    lib.tomo_lo_apply.argtypes = [vp, fp, fp, C.c_int, vp]
+    lib.tomo_lo_destroy.argtypes = [vp]
+    lib.tomo_lo_destroy.restype = None
     _lib = lib
     return lib
 
@@ -183,6 +191,17 @@ def host_structure_function(r, r0: float, L0: float) -> np.ndarray:
     return out.reshape(np.shape(r))
 
 
+def host_lo_estimator(cfg, sigma2_lo: float, slope_model: int = TOMO_HUDGIN, subap_mask=None):
+    """(R_lo [2T][2 n_lo], covariance of the aperture-mean slope pairs [2M][2M]) of tomo_host_lo_estimator."""
+    lib = load()
+    pr = _Problem(cfg, subap_mask)
+    n_lo, T = len(cfg.lo_wfs), len(cfg.targets)
+    R = np.empty((2 * T, 2 * n_lo), dtype=np.float64)
+    Cm = np.empty((2 * (n_lo + T), 2 * (n_lo + T)), dtype=np.float64)
+    _check(lib.tomo_host_lo_estimator(pr.geom, pr.cn2, cfg.r0, cfg.L0, slope_model, sigma2_lo, _dp(R), _dp(Cm)))
+    return R, Cm
+
+
 def measure_device(l2_bytes: int = 0, reps: int = 5, stream=None):
     """L2 -> SM read bandwidth [GB/s] and plain fp32 FMA rate [TFLOP/s] of the current device (tomo_measure_device)."""
     lib = load()
@@ -210,6 +229,37 @@ def _stream_handle(stream) -> int:
     import torch
     s = stream if stream is not None else torch.cuda.current_stream()
     return s.cuda_stream
+
+
+class LowOrder:
+    """tomo_lo_create / tomo_lo_apply / tomo_lo_destroy: the split low-order path of cfg.lo_wfs (include/tomo.h)."""
+
+    def __init__(self, cfg, sigma2_lo: float, slope_model: int = TOMO_HUDGIN, subap_mask=None):
+        self.lib = load()
+        self._pr = _Problem(cfg, subap_mask)
+        self.n_lo, self.n_targets = len(cfg.lo_wfs), len(cfg.targets)
+        self._h = C.c_void_p()
+        _check(self.lib.tomo_lo_create(self._pr.geom, self._pr.cn2, cfg.r0, cfg.L0, slope_model, sigma2_lo,
+                                       C.byref(self._h)))
+
+    def apply(self, lo_slopes, wavefront, stream=None):
+        """wavefront [n_frames][T][n_vphi] += tilt estimated from lo_slopes [n_frames][n_lo][2]; in place, asynchronous."""
+        n_frames = lo_slopes.shape[0] if lo_slopes.dim() == 3 else 1
+        if lo_slopes.numel() != n_frames * self.n_lo * 2 or wavefront.numel() % max(n_frames * self.n_targets, 1):
+            raise ValueError("lo_slopes must be [n_frames][n_lo][2] and wavefront [n_frames][T][n_vphi]")
+        _check(self.lib.tomo_lo_apply(self._h, _ptr(lo_slopes), _ptr(wavefront), n_frames, _stream_handle(stream)))
+        return wavefront
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            self.lib.tomo_lo_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
 
 class TomoPlan:
