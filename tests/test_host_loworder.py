@@ -61,3 +61,23 @@ def test_host_estimator_argument_errors():
     with pytest.raises(tomo.TomoError) as e:                  # two coincident noiseless sensors: singular C_gg
         tomo.host_lo_estimator(replace(cfg, lo_wfs=(LO3[0], LO3[0])), 0.0)
     assert e.value.code == tomo.TOMO_EINVAL
+
+
+def test_host_estimator_cfg4_full_size_properties():
+    """cfg4 (74 x 74, 3 NGS tip/tilt sensors, 10 targets, 35 layers): too large for the pair-by-pair oracle, so properties that
+    hold at any size: the covariance of the mean slopes is symmetric positive definite with equal diagonal blocks (every
+    direction sees the same statistics), R_lo C_gg-weighted gains stay below one, and with no noise a target placed on a
+    sensor takes that sensor's measurement."""
+    cfg = get_config("cfg4")
+    R, Cm = tomo.host_lo_estimator(cfg, 0.05)
+    assert R.shape == (2 * len(cfg.targets), 2 * len(cfg.lo_wfs))
+    assert np.abs(Cm - Cm.T).max() <= 1e-12 * np.abs(Cm).max()
+    assert np.linalg.eigvalsh(Cm).min() > 0
+    d0 = Cm[0:2, 0:2]
+    for k in range(Cm.shape[0] // 2):
+        assert np.allclose(Cm[2 * k:2 * k + 2, 2 * k:2 * k + 2], d0, rtol=1e-12, atol=1e-14 * np.abs(d0).max())
+    gains = R[0::2, 0::2].sum(axis=1)              # x-tilt of each target from the x-slopes of all sensors
+    assert np.all(gains > 0.0) and np.all(gains < 1.0)
+    s0 = cfg.lo_wfs[0]
+    R0, _ = tomo.host_lo_estimator(replace(cfg, lo_wfs=(s0,), targets=((s0.ax, s0.ay),)), 0.0)
+    assert np.allclose(R0, np.eye(2), atol=1e-10)
