@@ -61,3 +61,29 @@ def test_lo_apply_zero_frames_and_bad_arguments():
     with pytest.raises(ValueError):
         lo.apply(torch.ones((2, 2, 2), dtype=torch.float32, device="cuda"), torch.ones((2, 1, 69), dtype=torch.float32, device="cuda"))
     lo.close()
+
+
+def test_lo_apply_full_size_cfg4_batch16():
+    """cfg4 geometry (4453 valid phase points, 10 targets, 3 sensors), 16 frames: every output against the oracle's add-back.
+    The pair-by-pair oracle cannot build R_lo at this size, so R_lo here is the library's host builder's (gated against the
+    oracle at small sizes and by its full-size properties in tests/test_host_loworder.py); the kernel under test only applies it."""
+    import torch
+    from paper_1806_07938_b200 import tomo
+    cfg = get_config("cfg4")
+    d = cfg.D / cfg.n
+    sm = geo.subap_mask(cfg.n, cfg.D, cfg.obstruction)
+    pts = geo.phase_points(cfg.n, d)[geo.phase_mask(sm).ravel()]
+    R, _ = tomo.host_lo_estimator(cfg, 0.05)
+    rng = np.random.default_rng(BASE_SEED + 404)
+    n_frames, T, n_lo = 16, len(cfg.targets), len(cfg.lo_wfs)
+    g = rng.standard_normal((n_frames, n_lo, 2))
+    w0 = rng.standard_normal((n_frames, T, pts.shape[0]))
+    want = w0 + np.stack([olo.lo_addback(R, g[f], pts) for f in range(n_frames)])
+    lo = tomo.LowOrder(cfg, 0.05)
+    wd = torch.tensor(w0, dtype=torch.float32, device="cuda")
+    lo.apply(torch.tensor(g, dtype=torch.float32, device="cuda"), wd)
+    torch.cuda.synchronize()
+    got = wd.cpu().numpy().astype(np.float64)
+    lo.close()
+    assert got.shape == want.shape
+    assert np.abs(got - want).max() <= 2e-6 * np.abs(want).max()
