@@ -46,9 +46,10 @@ extern "C" {
 #define TOMO_F64       2       /* everything fp64 (parity gate P-e); the slope / wavefront ABI stays fp32             */
 
 #define TOMO_SOLVER_MULTIKERNEL 0   /* one kernel per phase, whole solve replayed from a CUDA graph                  */
-#define TOMO_SOLVER_PERSISTENT  1   /* one cooperative persistent kernel per solve, device-side grid barriers;       */
-                                    /* falls back to the multi-kernel solver where it does not apply (FFT edge not   */
-                                    /* instantiated, non-uniform noise diagonal)                                     */
+#define TOMO_SOLVER_PERSISTENT  1   /* one cooperative persistent kernel per solve, device-side grid exchanges.      */
+                                    /* Where it does not apply (FFT edge not instantiated, non-uniform or 2 x 2      */
+                                    /* block noise) tomo_plan_upload_kernels selects the multi-kernel solver instead, */
+                                    /* once, and tomo_get_solver reports which one runs and why                      */
 
 typedef struct tomo_plan tomo_plan;          /* opaque; owns every device allocation it makes                        */
 
@@ -134,7 +135,9 @@ int tomo_solve_minres(tomo_plan *plan, const float *slopes, float *wavefront_out
                       const float *x0, void *cuda_stream);
 
 /* out = M_s (W_s Sigma_ss W_s^T + Sigma_eta) M_s^T v  (Eq.30, Eq.34): one product, for the MVM gate.
- * v, out: device fp32 [C][n_vs]. */
+ * Computed by the solver that runs the plan's solves (tomo_get_solver): with the persistent solver it is ONE launch of the
+ * persistent kernel in its single-product mode (the same phase code, instance and shared-memory layout as a solve), else
+ * the multi-kernel product.  v, out: device fp32 [C][n_vs]. */
 int tomo_apply_css(tomo_plan *plan, const float *v, float *out, void *cuda_stream);
 
 /* wavefront_out = M_phi W_phi Sigma_{phi s} W_s^T M_s^T zeta  (Eq.31/32, Eq.35) for every target (A7-A8 only).
@@ -192,6 +195,11 @@ int tomo_get_noise(const tomo_plan *plan, double *sigma2_wfs, double *slope_var)
 /* Residual history sqrt(rho_k), k = 0..n_iter of the last solve: host fp64 [n_frames][n_iter+1].  The caller
  * must have synchronised the stream of that solve; this call copies device->host synchronously. */
 int tomo_get_residuals(const tomo_plan *plan, double *host_out, int n_frames, int n_iter);
+
+/* The solver that runs this plan's solves, products and CG steps (TOMO_SOLVER_*), decided once by
+ * tomo_plan_upload_kernels (TOMO_ENOTREADY before it), and -- when TOMO_SOLVER_PERSISTENT was asked for but does not apply --
+ * the reason, copied as a NUL-terminated string into note (host, note_cap bytes; may be NULL).  Never changes afterwards. */
+int tomo_get_solver(const tomo_plan *plan, int *solver_in_use, char *note, int note_cap);
 
 /* Bytes of device memory owned by the plan, and the number of kernel launches the last solve enqueued. */
 int tomo_get_stats(const tomo_plan *plan, long long *device_bytes, int *launches_last_solve);

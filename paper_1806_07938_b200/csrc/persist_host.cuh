@@ -25,8 +25,7 @@ struct PersistState {
     int off_ms2 = 0, fb = 1;
     size_t smem = 0;
     bool attr_set = false, attr_set_batch = false;
-    int *d_seg = nullptr;        // [F_max + 1][sms][8] slab segment tables, one per frame count (slab_segments)
-    std::vector<char> seg_ready; // table for n_frames = f uploaded?
+    int *d_seg = nullptr;        // [F_max + 1][sms][8] slab segment tables, one per frame count (slab_segments), uploaded by persist_prepare
     int sms = 0;
 };
 
@@ -69,13 +68,6 @@ static int persist_launch(tomo_plan *pl, cudaStream_t st, const PLaunch &L) {
     a.off_tab = ps->off_tab; a.off_upart = ps->off_upart; a.off_vm = ps->off_vm; a.off_vec = ps->off_vec;
     a.off_spec = ps->off_spec; a.off_ptab = ps->off_ptab; a.off_unit = ps->off_unit; a.ngs = ps->ngs;
     a.off_ms2 = ps->off_ms2; a.fb = ps->fb;
-    if (!ps->seg_ready[L.F]) {
-        std::vector<int> seg;
-        slab_segments(m.Ph, L.F, a.G, seg);
-        PCK(cudaMemcpyAsync(ps->d_seg + (size_t)L.F * ps->sms * 8, seg.data(), seg.size() * sizeof(int), cudaMemcpyHostToDevice, st));
-        PCK(cudaStreamSynchronize(st));          // the host vector goes out of scope; once per frame count
-        ps->seg_ready[L.F] = 1;
-    }
     a.seg = ps->d_seg + (size_t)L.F * ps->sms * 8;
     a.s_in = L.slopes; a.x0 = L.x0;
     a.x = (T *)pl->d_x; a.r = (T *)pl->d_r; a.p = (T *)pl->d_p;

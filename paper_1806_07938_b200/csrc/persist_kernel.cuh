@@ -40,7 +40,7 @@ static const int kPThreads = 512;
 static const int kPWarps = kPThreads / 32;
 static const int kGS = 16;                       // lanes per row unit
 
-enum { PM_COLD = 0, PM_WARM = 1, PM_STATE = 2 };
+enum { PM_COLD = 0, PM_WARM = 1, PM_STATE = 2, PM_APPLY = 3 };   // PM_APPLY: one product, r <- M_s A M_s v (tomo_apply_css)
 enum { PT_START = 0, PT_RHO = 1, PT_BUILD = 2, PT_FFT = 3, PT_MAC = 4, PT_INV = 5, PT_BAR_B = 6, PT_SCAL = 7, PT_ROWS = 8, PT_BAR_A = 9, PT_R_LOAD = 10, PT_R_FFT1 = 11, PT_R_UPD = 12, PT_R_FFT2 = 13, PT_N = 16 };
 
 // per-frame scalar block in shared memory (doubles)
@@ -741,7 +741,8 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                 const double rho_k = sc[SC_RHO], pq_k = sc[SC_PQ];
                 const double al = (!pre && rho_k > 0.0 && pq_k > 0.0) ? div_as<T>(rho_k, pq_k) : 0.0;   // = sc[SC_ALPHA]
                 const T alpha = (T)al, beta = (T)sc[SC_BETA];
-                const bool upd = sc[SC_UPD] != 0.0, step = al != 0.0;
+                const bool apply = a.mode == PM_APPLY;
+                const bool upd = sc[SC_UPD] != 0.0, step = al != 0.0 && !apply;
                 // mode coefficients (Z^T Z)^-1 Z^T q of this unit's WFS from the channel sums (Eq.36)
                 T c0 = (T)0, c2 = (T)0;
                 {
@@ -795,6 +796,9 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                                         if (pre) {                                   // warm start: r = b - M_s q, p = r
                                             rv = rv_[mm][row] - qp;
                                             ur[idx] = rv; up[idx] = rv;
+                                        } else if (apply) {                   // one product: r <- q' = M_s q
+                                            rv = qp;
+                                            ur[idx] = rv;
                                         } else {
                                             rv = rv_[mm][row];
                                             T pv = pv_[mm][row];

@@ -172,8 +172,17 @@ static int persist_prepare(tomo_plan *pl) {
     const size_t dsz = (size_t)F * m.C * 2 * npairs * m.n * E;
     PTRY(palloc(pl, (void **)&ps->d_flags, 1024));
     ps->sms = sms;
-    ps->seg_ready.assign((size_t)F + 1, 0);
     PTRY(palloc(pl, (void **)&ps->d_seg, (size_t)(F + 1) * sms * 8 * sizeof(int)));
+    {   // slab work tables of every frame count a solve may be given: the solve path itself never synchronises with the host
+        std::vector<int> all((size_t)(F + 1) * sms * 8, 0), seg;
+        for (int f = 1; f <= F; ++f) {
+            const int Gf = std::max(1, std::min(ps->G, std::max(f * U, m.Ph)));
+            slab_segments(m.Ph, f, Gf, seg);
+            std::copy(seg.begin(), seg.end(), all.begin() + (size_t)f * sms * 8);
+        }
+        cudaError_t e = cudaMemcpy(ps->d_seg, all.data(), all.size() * sizeof(int), cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) { delete ps; set_error(std::string("cudaMemcpy: ") + cudaGetErrorString(e)); return TOMO_ECUDA; }
+    }
     PTRY(palloc(pl, &ps->d_T1, tsz));
     PTRY(palloc(pl, &ps->d_T1p, tsz));
     PTRY(palloc(pl, &ps->d_T2, tsz));
@@ -234,6 +243,19 @@ int solve_persistent(tomo_plan *pl, const float *slopes, float *out, int F, int 
     pl->last_frames = F; pl->last_iter = n_iter;
     return TOMO_OK;
 }
+
+// one product through the persistent kernel (tomo_apply_css with the persistent solver): r <- M_s (W Sigma_ss W^T + Sigma_eta) M_s^T v
+int vec_store(tomo_plan *pl, cudaStream_t st, const void *src, float *dst);
+int apply_css_persistent(tomo_plan *pl, const float *v, float *out, cudaStream_t st) {
+    int rc;
+    if ((rc = persist_prepare(pl))) return rc;
+    pl->launches_last = 0;
+    if ((rc = persist_dispatch(pl, st, 1, 1, PM_APPLY, 0, v, nullptr, nullptr))) return rc;
+    return vec_store(pl, st, pl->d_r, out);
+}
+
+// decided once, when the spectra are uploaded: can the persistent solver run this plan?  (TOMO_EUNSUPPORTED = no)
+int persist_prepare_plan(tomo_plan *pl) { return persist_prepare(pl); }
 
 // one teacher-forced iteration through the persistent kernel (tomo_cg_step with the persistent solver)
 int cg_step_persistent(tomo_plan *pl, float *x, float *r, float *p, double *scal, cudaStream_t st) {

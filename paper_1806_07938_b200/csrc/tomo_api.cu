@@ -78,7 +78,10 @@ using namespace tomo;
 
 extern "C" const char *tomo_last_error(void) { return g_err.c_str(); }
 
-namespace tomo { void persist_destroy(tomo_plan *pl); }
+namespace tomo {
+void persist_destroy(tomo_plan *pl);
+int persist_prepare_plan(tomo_plan *pl);
+}
 
 extern "C" void tomo_plan_destroy(tomo_plan *pl) {
     if (!pl) return;
@@ -237,7 +240,19 @@ static int upload_kernels_impl(tomo_plan *pl, const double *css_gen, const doubl
 extern "C" int tomo_plan_upload_kernels(tomo_plan *pl, const double *css_gen, const double *cos_gen) {
     if (!pl) { set_error("plan is NULL"); return TOMO_EINVAL; }
     CK(cudaSetDevice(pl->device));
-    return pl->selem == 8 ? upload_kernels_impl<double>(pl, css_gen, cos_gen) : upload_kernels_impl<float>(pl, css_gen, cos_gen);
+    int rc = pl->selem == 8 ? upload_kernels_impl<double>(pl, css_gen, cos_gen) : upload_kernels_impl<float>(pl, css_gen, cos_gen);
+    if (rc) return rc;
+    // which solver runs this plan is decided HERE, once (never inside a solve): the persistent kernel where it applies,
+    // else the multi-kernel solver, with the reason kept for tomo_get_solver
+    pl->solver_used = TOMO_SOLVER_MULTIKERNEL;
+    pl->solver_note.clear();
+    if (pl->opt.solver == TOMO_SOLVER_PERSISTENT) {
+        rc = persist_prepare_plan(pl);
+        if (rc == TOMO_OK) pl->solver_used = TOMO_SOLVER_PERSISTENT;
+        else if (rc == TOMO_EUNSUPPORTED) pl->solver_note = g_err;
+        else return rc;
+    }
+    return TOMO_OK;
 }
 
 // ------------------------------------------------------------------------------------------------ launch sequences
@@ -701,6 +716,14 @@ template <typename T, typename S> struct Ops {
         return TOMO_OK;
     }
 
+    static int vec_store(tomo_plan *pl, cudaStream_t st, const void *src, float *dst) {
+        const size_t cnt = (size_t)pl->m.C * pl->m.nv;
+        k_convert<T, float><<<(unsigned)std::min<size_t>((cnt + 255) / 256, 148 * 8), 256, 0, st>>>((const T *)src, dst, cnt);
+        LAUNCH_CHECK();
+        pl->launches_last += 1;
+        return TOMO_OK;
+    }
+
     static int get_zeta(tomo_plan *pl, float *out, int F, cudaStream_t st) {
         const size_t cnt = (size_t)F * pl->m.C * pl->m.nv;
         k_convert<T, float><<<(unsigned)std::min<size_t>((cnt + 255) / 256, 148 * 8), 256, 0, st>>>((const T *)pl->d_x, out, cnt);
@@ -736,6 +759,8 @@ int state_load(tomo_plan *pl, cudaStream_t st, const float *x, const float *r, c
     return DISPATCH(pl, state_load(pl, st, x, r, p, rho));
 }
 int state_store(tomo_plan *pl, cudaStream_t st, float *x, float *r, float *p) { return DISPATCH(pl, state_store(pl, st, x, r, p)); }
+int vec_store(tomo_plan *pl, cudaStream_t st, const void *src, float *dst) { return DISPATCH(pl, vec_store(pl, st, src, dst)); }
+int apply_css_persistent(tomo_plan *pl, const float *v, float *out, cudaStream_t st);
 }  // namespace tomo
 
 extern "C" int tomo_solve_batch(tomo_plan *pl, const float *slopes, float *wavefront_out, int n_frames, int n_iter,
@@ -747,12 +772,7 @@ extern "C" int tomo_solve_batch(tomo_plan *pl, const float *slopes, float *wavef
     if (n_iter < 0 || n_iter >= pl->hist_cap) { set_error("n_iter outside [0, 1024]"); return TOMO_EINVAL; }
     if (pl->has_cos && !wavefront_out) { set_error("wavefront_out is NULL"); return TOMO_EINVAL; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    if (pl->opt.solver == TOMO_SOLVER_PERSISTENT) {
-        // FFT edges the persistent kernel is not instantiated for, non-uniform noise, ...: the multi-kernel solver takes over
-        rc = solve_persistent(pl, slopes, wavefront_out, n_frames, n_iter, x0, st);
-        if (rc != TOMO_EUNSUPPORTED) return rc;
-        pl->opt.solver = TOMO_SOLVER_MULTIKERNEL;
-    }
+    if (pl->solver_used == TOMO_SOLVER_PERSISTENT) return solve_persistent(pl, slopes, wavefront_out, n_frames, n_iter, x0, st);
     return DISPATCH(pl, solve(pl, slopes, wavefront_out, n_frames, n_iter, x0, st));
 }
 
@@ -775,6 +795,8 @@ extern "C" int tomo_apply_css(tomo_plan *pl, const float *v, float *out, void *c
     int rc = check_ready(pl);
     if (rc) return rc;
     if (!v || !out) { set_error("NULL vector"); return TOMO_EINVAL; }
+    // the product of the solver that runs the solves: one single-product launch of the persistent kernel, or the multi-kernel product
+    if (pl->solver_used == TOMO_SOLVER_PERSISTENT) return apply_css_persistent(pl, v, out, (cudaStream_t)cuda_stream);
     return DISPATCH(pl, apply_css(pl, v, out, (cudaStream_t)cuda_stream));
 }
 
@@ -790,11 +812,7 @@ extern "C" int tomo_cg_step(tomo_plan *pl, float *x, float *r, float *p, double 
     int rc = check_ready(pl);
     if (rc) return rc;
     if (!x || !r || !p || !rho_alpha_beta) { set_error("NULL vector"); return TOMO_EINVAL; }
-    if (pl->opt.solver == TOMO_SOLVER_PERSISTENT) {
-        rc = cg_step_persistent(pl, x, r, p, rho_alpha_beta, (cudaStream_t)cuda_stream);
-        if (rc != TOMO_EUNSUPPORTED) return rc;
-        pl->opt.solver = TOMO_SOLVER_MULTIKERNEL;
-    }
+    if (pl->solver_used == TOMO_SOLVER_PERSISTENT) return cg_step_persistent(pl, x, r, p, rho_alpha_beta, (cudaStream_t)cuda_stream);
     return DISPATCH(pl, cg_step(pl, x, r, p, rho_alpha_beta, (cudaStream_t)cuda_stream));
 }
 
@@ -944,6 +962,14 @@ extern "C" int tomo_get_residuals(const tomo_plan *pl, double *host_out, int n_f
     CK(cudaMemcpy(h.data(), pl->d_hist, h.size() * sizeof(double), cudaMemcpyDeviceToHost));
     for (int f = 0; f < n_frames; ++f)
         for (int k = 0; k <= n_iter; ++k) host_out[(size_t)f * (n_iter + 1) + k] = std::sqrt(h[(size_t)f * pl->hist_cap + k]);
+    return TOMO_OK;
+}
+
+extern "C" int tomo_get_solver(const tomo_plan *pl, int *solver_in_use, char *note, int note_cap) {
+    if (!pl) { set_error("plan is NULL"); return TOMO_EINVAL; }
+    if (!pl->ready) { set_error("tomo_plan_upload_kernels has not been called"); return TOMO_ENOTREADY; }
+    if (solver_in_use) *solver_in_use = pl->solver_used;
+    if (note && note_cap > 0) { std::strncpy(note, pl->solver_note.c_str(), (size_t)note_cap - 1); note[note_cap - 1] = 0; }
     return TOMO_OK;
 }
 

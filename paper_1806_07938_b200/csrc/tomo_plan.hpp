@@ -50,6 +50,8 @@ struct tomo_plan {
     std::map<std::tuple<int, int, int>, int> graph_launches;   // kernel nodes in each cached graph
     std::vector<cudaEvent_t> *prof = nullptr;   // when set, launch sequences bracket every kernel with events
     void *persist = nullptr;     // persistent-solver state (solve_persistent.cu)
+    int solver_used = 0;         // TOMO_SOLVER_* that actually runs the solves: decided once, in tomo_plan_upload_kernels
+    std::string solver_note;     // why the persistent solver was not taken (empty when it was, or was not asked for)
 };
 
 namespace tomo {

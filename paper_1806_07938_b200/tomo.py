@@ -25,7 +25,7 @@ EXPORTS = (
     "tomo_plan_create", "tomo_plan_upload_kernels", "tomo_solve", "tomo_solve_batch", "tomo_solve_minres", "tomo_apply_css",
     "tomo_apply_cos", "tomo_cg_step", "tomo_get_zeta", "tomo_time_kernels", "tomo_time_phases", "tomo_time_solver", "tomo_measure_device",
     "tomo_get_sizes", "tomo_get_valid_index", "tomo_get_noise",
-    "tomo_get_residuals", "tomo_get_stats", "tomo_plan_destroy", "tomo_last_error",
+    "tomo_get_residuals", "tomo_get_stats", "tomo_get_solver", "tomo_plan_destroy", "tomo_last_error",
     "tomo_host_sizes", "tomo_host_css_generators", "tomo_host_cos_generators", "tomo_host_generator_spectrum",
     "tomo_host_structure_function", "tomo_host_slab_segments",
     "tomo_host_lo_estimator", "tomo_lo_create", "tomo_lo_apply", "tomo_lo_destroy",
@@ -98,6 +98,7 @@ def load(build_if_missing: bool = True):
     lib.tomo_get_noise.argtypes = [vp, dp, dp]
     lib.tomo_get_residuals.argtypes = [vp, dp, C.c_int, C.c_int]
     lib.tomo_get_stats.argtypes = [vp, C.POINTER(C.c_longlong), ip]
+    lib.tomo_get_solver.argtypes = [vp, ip, C.c_char_p, C.c_int]
     lib.tomo_plan_destroy.argtypes = [vp]
     lib.tomo_plan_destroy.restype = None
     lib.tomo_host_sizes.argtypes = [C.POINTER(_Geometry), C.POINTER(_Cn2), C.c_int, C.c_int, ip, ip, ip, ip, ip, ip]
@@ -367,6 +368,13 @@ class TomoPlan:
         n = C.c_int()
         _check(self.lib.tomo_get_stats(self._h, C.byref(b), C.byref(n)))
         return dict(device_bytes=b.value, launches_last_solve=n.value)
+
+    def solver_in_use(self):
+        """(TOMO_SOLVER_* that runs this plan, reason the persistent solver was not taken or '')."""
+        sv = C.c_int()
+        note = C.create_string_buffer(512)
+        _check(self.lib.tomo_get_solver(self._h, C.byref(sv), note, 512))
+        return sv.value, note.value.decode()
 
     # -- convenience: host buffers in, host buffers out (H2D + solve + D2H on one stream) --
     def solve_host(self, slopes_host, n_iter: int, n_frames: int = 1, stream=None, minres: bool = False):
