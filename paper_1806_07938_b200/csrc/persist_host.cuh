@@ -4,6 +4,7 @@
 #include <algorithm>
 #include <cstring>
 #include <string>
+#include <type_traits>
 #include <vector>
 
 #include "tomo.h"
@@ -24,7 +25,7 @@ struct PersistState {
     int off_ms = 0, off_work = 0, off_red = 0, off_scal = 0, off_tab = 0, off_upart = 0, off_vm = 0, off_vec = 0, off_spec = 0, off_ptab = 0, off_unit = 0, ngs = 2;
     int off_ms2 = 0, fb = 1;
     size_t smem = 0;
-    bool attr_set = false, attr_set_batch = false;
+    bool attr_set = false, attr_set_batch = false, attr_set_prof = false, attr_set_prof_batch = false;
     int *d_seg = nullptr;        // [F_max + 1][sms][8] slab segment tables, one per frame count (slab_segments), uploaded by persist_prepare
     int sms = 0;
 };
@@ -78,8 +79,14 @@ static int persist_launch(tomo_plan *pl, cudaStream_t st, const PLaunch &L) {
     a.part_r = ps->d_part_r; a.part_s = ps->d_part_s; a.part_i = ps->d_part_i;
     a.hist = pl->d_hist; a.hist_stride = pl->hist_cap; a.alpha = pl->d_alpha; a.scal_out = L.scal_out;
     a.flags = ps->d_flags; a.dbg = L.dbg;
-    const void *kern = L.F > 1 ? (const void *)(k_persistent<T, S, P, true>) : (const void *)(k_persistent<T, S, P, false>);
-    bool &attr_set = L.F > 1 ? ps->attr_set_batch : ps->attr_set;
+    // the instrumented instances (tomo_time_phases) exist for TOMO_F32 only; the production instances carry no stamp code
+    const void *kern = L.F > 1 ? (const void *)(k_persistent<T, S, P, true, false>) : (const void *)(k_persistent<T, S, P, false, false>);
+    if (L.dbg) {
+        if constexpr (std::is_same<T, float>::value && std::is_same<S, float>::value)
+            kern = L.F > 1 ? (const void *)(k_persistent<T, S, P, true, true>) : (const void *)(k_persistent<T, S, P, false, true>);
+        else { set_error("tomo_time_phases: the instrumented kernel instances exist for TOMO_F32 only"); return TOMO_EUNSUPPORTED; }
+    }
+    bool &attr_set = L.dbg ? (L.F > 1 ? ps->attr_set_prof_batch : ps->attr_set_prof) : (L.F > 1 ? ps->attr_set_batch : ps->attr_set);
     if (!attr_set) {
         PCK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ps->smem));
         int occ = 0;

@@ -280,8 +280,9 @@ template <typename T> __device__ __forceinline__ double warp_sum_red(const T *sr
 }
 
 // BATCH = false: the single-frame instance (latency-bound: compact code, the CTA's own slab only);
-// BATCH = true: several frames per solve (throughput: balanced slab passes, every global load of a step issued up front)
-template <typename T, typename S, int P, bool BATCH>
+// BATCH = true: several frames per solve (throughput: balanced slab passes, every global load of a step issued up front).
+// PROF = true: thread 0 stamps clock64 at the phase boundaries (tomo_time_phases); the production instances carry no stamp code.
+template <typename T, typename S, int P, bool BATCH, bool PROF>
 __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
     typedef typename cx_of<T>::type C2;
     typedef typename cx_of<S>::type S2;
@@ -315,7 +316,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
     unsigned epoch = 0;
     const T half_n = (T)(0.5 * (n - 1)), dd = (T)a.g.d;
     int k = -2;                                      // iteration index seen by PSTAMP (no stamps outside the loop)
-#define PSTAMP(pt) do { if (a.dbg && tid == 0 && k >= 0) a.dbg[((size_t)b * a.n_iter + k) * PT_N + (pt)] = clock64(); } while (0)
+#define PSTAMP(pt) do { if (PROF) { if (a.dbg && tid == 0 && k >= 0) a.dbg[((size_t)b * a.n_iter + k) * PT_N + (pt)] = clock64(); } } while (0)
 #define GRID_SYNC() do { epoch += G; grid_sync(a.flags, epoch); } while (0)
 
     // ---- slab ownership: CTA b owns k_x = b % Ph and a contiguous share of the frames
