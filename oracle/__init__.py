@@ -11,7 +11,8 @@ What it computes (each module cites the passage it follows, PAPER.md L<line>):
   geometry.py    subaperture / phase-point grids, pupil masks (Fig.2)
   covariance.py  linear-stencil slope models (Eq.47-48, Eq.54-55), dense C_ss (Eq.14,
                  L136-158) and C_os (Eq.15-17, L170-197) built from POSITIONS
-  fftmodel.py    FFT slope model Eq.41-46 (L534-572) as a direct Riemann sum over the FFT's frequency grid
+  fftmodel.py    FFT slope model Eq.41-46 (L534-572): the continuous integrals, evaluated in physical space (edge-averaged
+                 structure function, Gauss-Legendre panels); shares no grid with the library's FFT-based builder
   projectors.py  W, Z, M = I - Z Z^+ (Eq.33-36)
   solver.py      direct solve of Eq.5/Eq.12, textbook CG and MINRES (S2.G L337, L426), Eq.13
   toeplitz.py    the paper's 2RBT product Eq.18-28 step by step, generators, op counts
@@ -26,7 +27,8 @@ stencil evaluation, symmetry/PSD of C_ss, dense == paper's index maps == 2-D FFT
 product, projector identities, CG -> Cholesky, MINRES = the least-squares minimiser over the
 Krylov space (brute force) = scipy's minres, LGS ground-layer identity, the
 paper's printed closed-form counts (L150, L177, L197, L270, L280, L295), the telescoping
-closed form of the aperture-mean Hudgin slope variance (loworder.py).
+closed form of the aperture-mean Hudgin slope variance (loworder.py); the FFT slope model against Eq.43 / Eq.46 as
+printed, summed over frequency grids refined to convergence, and against adaptive quadrature (test_oracle_fftmodel.py).
 
 Parity unpinned: absolute WFE in nm (Table 3) and the curves of Fig.9-15 are not
 reproduced; nothing in this package depends on them.

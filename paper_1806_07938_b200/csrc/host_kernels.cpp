@@ -65,10 +65,15 @@ const int kFftOver = 4;
 const double kPsdConst = std::pow(24.0 * std::tgamma(6.0 / 5.0) / 5.0, 5.0 / 6.0) * std::tgamma(11.0 / 6.0) * std::tgamma(11.0 / 6.0) /
                          (2.0 * std::pow(M_PI, 11.0 / 3.0));
 
-int fft_grid_edge(int max_lag) {                      // power of two, >= 512, lags up to max_lag representable
+// Edge of the FFT grid (pixel w / kFftOver): a power of two >= 512 whose period NG w / kFftOver holds the largest separation
+// the table is read at -- |lag| w PLUS the guide-star / target shift h_k d_alpha that enters as a phase ramp -- with at least
+// one outer scale to the nearest alias (the table is the covariance periodised with that period; beyond L0 the slope
+// covariances have decayed to < 1e-3 of the variance)
+int fft_grid_edge(int max_lag, double w, double shx, double shy, double L0) {
+    const double need = max_lag * w + std::max(std::fabs(shx), std::fabs(shy)) + L0;      // [m]
     int ng = 512;
-    while (kFftOver * max_lag >= ng / 2) ng *= 2;
-    return ng;
+    while (ng * w / kFftOver < need || kFftOver * max_lag >= ng / 2) ng *= 2;
+    return std::min(ng, 8192);
 }
 double sinc_pi(double x) { return x == 0.0 ? 1.0 : std::sin(M_PI * x) / (M_PI * x); }
 
@@ -104,9 +109,10 @@ double model_slope_variance(const HostModel &m) {
     double v = 0.0;
     const double c = 1.0 / m.d;
     if (m.slope_model == TOMO_FFTMODEL) {
-        const int NG = fft_grid_edge(m.n_p);
         for (int k = 0; k < m.K; ++k) {
-            const double w = m.gamma[k] * m.d, df = kFftOver / (NG * w);
+            const double w = m.gamma[k] * m.d;
+            const int NG = fft_grid_edge(m.n_p, w, 0.0, 0.0, m.L0);
+            const double df = kFftOver / (NG * w);
             double s = 0.0;
             for (int py = -(NG / 2 - 1); py < NG / 2; ++py)
                 for (int px = -(NG / 2 - 1); px < NG / 2; ++px) {
@@ -155,7 +161,7 @@ void build_css_generators(const HostModel &m, std::vector<double> &gen) {
             const double w = m.gamma[k] * m.d;
             const double shx = m.h[k] * (m.ax[j] - m.ax[i]), shy = m.h[k] * (m.ay[j] - m.ay[i]);
             if (m.slope_model == TOMO_FFTMODEL) {
-                const int NG = fft_grid_edge(m.n_p);
+                const int NG = fft_grid_edge(n, w, shx, shy, m.L0);
                 std::vector<std::complex<double>> tab;
                 for (int a = 0; a < 2; ++a)
                     for (int b = a; b < 2; ++b) {
@@ -305,7 +311,7 @@ void build_cos_generators(const HostModel &m, int target, std::vector<double> &g
             const double shx = off + m.h[k] * (m.ax[j] - m.bx[target]);
             const double shy = off + m.h[k] * (m.ay[j] - m.by[target]);
             if (m.slope_model == TOMO_FFTMODEL) {
-                const int NG = fft_grid_edge(m.n_p);
+                const int NG = fft_grid_edge(m.n_p, w, shx, shy, m.L0);
                 std::vector<std::complex<double>> tab;
                 for (int b = 0; b < 2; ++b) {
                     fft_model_table(NG, w, m.gamma[k], m.r0, m.L0, shx, shy, 3 + b, tab);

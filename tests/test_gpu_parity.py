@@ -72,9 +72,33 @@ def system(name):
     return _cache[name]
 
 
+def _oracle_fft_generators(cfg, osys):
+    """Generators of the FFT slope model from the ORACLE (the continuous integrals of Eq.43 / Eq.46): css [C][C][2n-1][2n-1],
+    cos [T][K][C][n'+n-1][n'+n-1] in the layout of tomo_plan_upload_kernels."""
+    from oracle import toeplitz as tz
+    n, N = cfg.n, len(cfg.wfs)
+    css = tz.css_generators(n, cfg.d, osys.dirs, osys.h_gs, cfg.h, cfg.frac, cfg.r0, cfg.L0, "fft").reshape(2 * N, 2 * N, 2 * n - 1, 2 * n - 1)
+    cos = []
+    for beta in cfg.targets:
+        xi = tz.cos_generators(n, osys.n_p, cfg.d, osys.dirs, osys.h_gs, beta, cfg.h, cfg.frac, cfg.r0, cfg.L0, "fft")
+        cos.append(xi.reshape(xi.shape[0], 2 * N, xi.shape[-1], xi.shape[-1]))
+    return css, np.stack(cos)
+
+
 def make_plan(name, **kw):
     cfg, model, osys, _ = system(name)
     sm = {"fried": tomo.TOMO_FRIED, "fft": tomo.TOMO_FFTMODEL}.get(model, tomo.TOMO_HUDGIN)
+    if model == "fft":
+        # The oracle of the FFT slope model is the continuous integral; the library's builder evaluates it on a truncated
+        # frequency grid (0.13 % of the slope variance off, gated in tests/test_host_builder.py).  The KERNELS are compared with
+        # the oracle on the oracle's own generators (tomo_plan_upload_kernels takes them) and noise level;
+        # test_fft_model_plan_from_the_builder below covers the plan the builder makes.
+        if "fftgen" not in _cache:
+            _cache["fftgen"] = _oracle_fft_generators(cfg, osys)
+        css, cos = _cache["fftgen"]
+        pl = tomo.TomoPlan(cfg, slope_model=sm, sigma2_wfs=[osys.sigma2] * len(cfg.wfs), css_gen=css, cos_gen=cos, **kw)
+        assert pl.solver_in_use()[0] == kw.get("solver", tomo.TOMO_SOLVER_PERSISTENT), pl.solver_in_use()
+        return pl
     pl = tomo.TomoPlan(cfg, slope_model=sm, **kw)
     # every plan of this file runs on the solver it asks for (default: the persistent kernel); none may fall back silently
     assert pl.solver_in_use()[0] == kw.get("solver", tomo.TOMO_SOLVER_PERSISTENT), pl.solver_in_use()
@@ -83,6 +107,29 @@ def make_plan(name, **kw):
     sub, ph = pl.valid_index()
     assert np.array_equal(sub, osys.sub_idx) and np.array_equal(ph, osys.ph_idx)
     return pl
+
+
+def test_fft_model_plan_from_the_builder_is_within_its_discretisation_error():
+    """TOMO_FFTMODEL end to end with the BUILDER's generators (2-D FFTs on a grid cut at |f| < 2/w): product and converged
+    wavefront within 1 % of the continuous-integral oracle (the generators are 0.13 % of the variance off; G29)."""
+    cfg, model, osys, data = system("small_fftmodel")
+    pl = tomo.TomoPlan(cfg, slope_model=tomo.TOMO_FFTMODEL)
+    s2, var = pl.noise()
+    assert abs(var / osys.slope_var - 1) < 5e-3
+    s = f32(data["slopes"][0].ravel())
+    d_o = torch.empty(osys.Ns, dtype=torch.float32, device="cuda")
+    pl.apply_css(dev(s), d_o)
+    torch.cuda.synchronize()
+    assert rel(d_o.cpu().numpy(), osys.apply_A(s)) <= 1e-2
+    _, h = osys.solve_cg(s, 1000)
+    n_it = int(np.flatnonzero(h / h[0] < 1e-6)[0])
+    d_w = torch.empty(pl.wavefront_len, dtype=torch.float32, device="cuda")
+    pl.solve(dev(s), d_w, n_it)
+    torch.cuda.synchronize()
+    e = rel(d_w.cpu().numpy().reshape(len(cfg.targets), -1)[0], osys.reconstruct(osys.solve_direct(s), 0))
+    print(f"[FFT model, builder's generators] converged wavefront vs the continuous-integral oracle: {e:.2e}")
+    assert e <= 1e-2
+    pl.close()
 
 
 ALL = ["cfg1", "small_lgs", "small_odd_focus", "small_fried", "small_fftmodel", "ngs_offaxis", "cfg2"]

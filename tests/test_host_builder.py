@@ -61,26 +61,83 @@ def test_sizes_of_the_configs():
     assert [tomo.host_sizes(sweep_config(n))["n_prime"] for n in (16, 32, 64, 96, 128)] == [25, 47, 91, 135, 179]
 
 
-@pytest.mark.parametrize("model", [tomo.TOMO_HUDGIN, tomo.TOMO_FRIED, tomo.TOMO_FFTMODEL])
-@pytest.mark.parametrize("name", ["cfg1", "small_lgs"])
-def test_generators_match_oracle(name, model):
-    cfg = get_config("cfg1") if name == "cfg1" else small_lgs_config(n=9, n_gs=3, n_layers=3, targets=((5.0, -3.0),))
-    mname = {tomo.TOMO_HUDGIN: "hudgin", tomo.TOMO_FRIED: "fried", tomo.TOMO_FFTMODEL: "fft"}[model]
+def _oracle_generators(cfg, mname):
     dirs = [(w.ax, w.ay) for w in cfg.wfs]
     hgs = cfg.wfs[0].h_gs
     N, n = len(dirs), cfg.n
     th = tz.css_generators(n, cfg.d, dirs, hgs, cfg.h, cfg.frac, cfg.r0, cfg.L0, mname).reshape(2 * N, 2 * N, 2 * n - 1, 2 * n - 1)
-    g = tomo.host_css_generators(cfg, model)
-    # (FFT model: the builder's 2-D FFT against the oracle's direct Riemann sum over the same frequency grid)
-    assert np.abs(g - th).max() <= (1e-9 if model == tomo.TOMO_FFTMODEL else 1e-11) * np.abs(th).max()
     sz = tomo.host_sizes(cfg)
     xi = tz.cos_generators(n, sz["n_prime"], cfg.d, dirs, hgs, cfg.targets[0], cfg.h, cfg.frac, cfg.r0, cfg.L0, mname)
     if math.isinf(hgs):
         xi = xi.sum(axis=0, keepdims=True)        # NGS: layers share one grid and are summed (Eq.15)
-    xi = xi.reshape(xi.shape[0], 2 * N, xi.shape[-1], xi.shape[-1])
+    return th, xi.reshape(xi.shape[0], 2 * N, xi.shape[-1], xi.shape[-1])
+
+
+@pytest.mark.parametrize("model", [tomo.TOMO_HUDGIN, tomo.TOMO_FRIED])
+@pytest.mark.parametrize("name", ["cfg1", "small_lgs"])
+def test_generators_match_oracle(name, model):
+    cfg = get_config("cfg1") if name == "cfg1" else small_lgs_config(n=9, n_gs=3, n_layers=3, targets=((5.0, -3.0),))
+    th, xi = _oracle_generators(cfg, {tomo.TOMO_HUDGIN: "hudgin", tomo.TOMO_FRIED: "fried"}[model])
+    g = tomo.host_css_generators(cfg, model)
+    assert np.abs(g - th).max() <= 1e-11 * np.abs(th).max()
     g2 = tomo.host_cos_generators(cfg, 0, model)
     assert g2.shape == xi.shape
-    assert np.abs(g2 - xi).max() <= (1e-9 if model == tomo.TOMO_FFTMODEL else 1e-11) * np.abs(xi).max()
+    assert np.abs(g2 - xi).max() <= 1e-11 * np.abs(xi).max()
+
+
+@pytest.mark.parametrize("name", ["cfg1", "small_lgs"])
+def test_fft_model_generators_discretisation_error_against_the_continuous_oracle(name, monkeypatch):
+    """TOMO_FFTMODEL (Eq.41-46): the builder evaluates the Fourier integrals by 2-D FFTs on a grid of pixel w / 4, i.e. cut at
+    |f| < 2 / w.  (i) Its FFT machinery reproduces the same Riemann sum written out directly (tests/fourier_sum.py) to 1e-9.
+    (ii) Against the ORACLE -- the continuous integral, evaluated in physical space, sharing no grid with the builder -- the
+    error is the truncated tail of sinc^2: ~0.2 % of the slope variance whatever w, r0 (both scale as r0^-5/3 w^-1/3; DESIGN.md
+    G29); gated at 0.5 %."""
+    import fourier_sum as fs
+    from oracle import fftmodel as fm
+    cfg = get_config("cfg1") if name == "cfg1" else small_lgs_config(n=9, n_gs=3, n_layers=3, targets=((5.0, -3.0),))
+    g = tomo.host_css_generators(cfg, tomo.TOMO_FFTMODEL)
+    g2 = tomo.host_cos_generators(cfg, 0, tomo.TOMO_FFTMODEL)
+    th, xi = _oracle_generators(cfg, "fft")                                   # continuous integral
+    var = th[0, 0, cfg.n - 1, cfg.n - 1]
+    e_ss, e_ps = np.abs(g - th).max() / var, np.abs(g2 - xi).max() / np.abs(xi).max()
+    print(f"[FFT model, {name}] builder vs continuous oracle: Sigma_ss {e_ss:.2e} of the variance, Sigma_phi-s {e_ps:.2e} of its maximum")
+    assert e_ss <= 5e-3 and e_ps <= 5e-3
+    monkeypatch.setattr(fm, "cov_slope_slope", lambda d, a, b, w, c, r0, L0: fs.cov_slope_slope(d, a, b, w, c, r0, L0, 512, 4))
+    monkeypatch.setattr(fm, "cov_phase_slope", lambda d, b, w, c, r0, L0: fs.cov_phase_slope(d, b, w, c, r0, L0, 512, 4))
+    th_g, xi_g = _oracle_generators(cfg, "fft")                               # the same sum on the builder's grid
+    assert np.abs(g - th_g).max() <= 1e-9 * np.abs(th_g).max()
+    assert np.abs(g2 - xi_g).max() <= 1e-9 * np.abs(xi_g).max()
+
+
+def test_fft_model_generators_at_elt_geometry_against_the_continuous_oracle():
+    """cfg3 geometry (n = 74, d = 0.5135 m, two opposite LGS of the 45" ring, layers up to 25 km): the builder's grid edge is
+    1024 here (lags up to 73 plus the guide-star shift h_k d_alpha, which enters as a phase ramp, plus one outer scale to the
+    nearest alias).  Sampled lags of the cross-WFS blocks against the continuous oracle: same 0.5 % gate, no wrap-around."""
+    from dataclasses import replace
+    from oracle import fftmodel as fm
+    from oracle import geometry as geo
+    from tomo_inputs.configs import WFS
+    c3 = get_config("cfg3")
+    cfg = replace(c3, wfs=(WFS(45.0, 0.0, 90e3, 2), WFS(-45.0, 0.0, 90e3, 2)), h=(0.0, 12500.0, 25000.0), frac=(0.5, 0.3, 0.2))
+    g = tomo.host_css_generators(cfg, tomo.TOMO_FFTMODEL)
+    n, d = cfg.n, cfg.d
+    rng = np.random.default_rng(74)
+    lags = np.concatenate([[[0, 0], [n - 1, n - 1], [-(n - 1), 0], [1, 0], [0, -1]], rng.integers(-(n - 1), n, size=(25, 2))])
+    var = g[0, 0, n - 1, n - 1]
+    worst = 0.0
+    for (i, j) in ((0, 0), (0, 1)):
+        for a in range(2):
+            for b in range(2):
+                want = np.zeros(len(lags))
+                for hk, fk in zip(cfg.h, cfg.frac):
+                    gam = geo.cone_factor(hk, 90e3)
+                    sh = hk * (np.array([cfg.wfs[j].ax, cfg.wfs[j].ay]) - np.array([cfg.wfs[i].ax, cfg.wfs[i].ay])) * geo.ARCSEC
+                    delta = gam * d * lags.astype(np.float64) + sh[None, :]
+                    want += fk * fm.cov_slope_slope(delta, a, b, gam * d, 1.0 / d, cfg.r0, cfg.L0)
+                got = g[2 * i + a, 2 * j + b, lags[:, 1] + n - 1, lags[:, 0] + n - 1]
+                worst = max(worst, float(np.abs(got - want).max() / var))
+    print(f"[FFT model, cfg3 geometry, grid edge 1024] builder vs continuous oracle: {worst:.2e} of the variance")
+    assert worst <= 5e-3
 
 
 @pytest.mark.parametrize("P", [16, 20, 30, 48])
