@@ -36,7 +36,7 @@ def parse():
     ap.add_argument("--solver", default=os.environ.get("TOMO_SOLVER", "persistent"), choices=["multikernel", "persistent"])
     ap.add_argument("--precision", default="f32", choices=["f32", "f32s_f64a", "f64"])
     ap.add_argument("--method", default="cg", choices=["cg", "minres"],
-                    help="cg (north_star's solver, the headline) or minres (the paper's solver for the Toeplitz method; multi-kernel path)")
+                    help="cg (north_star's solver, the headline) or minres (the paper's solver for the Toeplitz method, same persistent kernel)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
 
@@ -98,18 +98,28 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------------ reference arm
-def oracle_setup(cfg, n_iter):
-    """The fp64 oracle, as it stands, on a bounded sample of the workload.  Returns (step, description, cores);
+def _oracle_generator_rows(job):
+    from oracle import toeplitz as tz
+    (n, d, dirs, h_gs, h, frac, r0, L0, model, i) = job
+    return tz.css_generators(n, d, dirs, h_gs, h, frac, r0, L0, model, wfs_rows=[i])
+
+
+def oracle_setup(cfg, n_iter, whole):
+    """The fp64 oracle, as it stands, on a bounded sample of the workload.  Returns (step, description, cores, extrapolated);
     step() runs the sample once and returns the seconds per reconstruction it implies.
-    ELT sizes: ONE full matrix-free direct-sum Sigma_ss product (oracle/directsum.c, OpenMP) is timed and multiplied
-    by n_iter (the target projection is left out); tiny/mid sizes: the dense oracle's full CG solve + projection."""
+    tiny / mid sizes: the dense oracle's full CG solve + projection.
+    ELT sizes, whole = True (the reference arm): the WHOLE step -- n_iter matrix-free direct-sum products (oracle/directsum.c,
+    OpenMP) inside the oracle's CG, then the matrix-free target projection; the oracle's generator table (its one-time setup,
+    like the library's plan build) is built once, one process per output WFS.
+    ELT sizes, whole = False (the cpu_baseline leg of the GPU arm, which must stay short): the median of five timed direct-sum
+    products, times n_iter -- an extrapolation, flagged as such; the projection is left out."""
     import numpy as np
     from oracle import directsum
     from oracle import toeplitz as tz
     from oracle.system import OracleSystem
+    from tomo_inputs import screens
     cores = len(os.sched_getaffinity(0))
     if 2 * cfg.n_wfs * cfg.n * cfg.n <= 6000:
-        from tomo_inputs import screens
         osys = OracleSystem(cfg)
         s = screens.generate(cfg, osys.sigma2)["slopes"].ravel()
 
@@ -118,8 +128,23 @@ def oracle_setup(cfg, n_iter):
             x, _ = osys.solve_cg(s, n_iter)
             osys.reconstruct(x, 0)
             return time.perf_counter() - t0
-        return step, f"dense fp64 oracle: full {n_iter}-iteration CG solve + projection", cores
+        return step, f"dense fp64 oracle: full {n_iter}-iteration CG solve + projection", cores, False
     osys = OracleSystem(cfg, dense=False)
+    if whole:
+        from concurrent.futures import ProcessPoolExecutor
+        jobs = [(cfg.n, cfg.d, osys.dirs, osys.h_gs, list(cfg.h), list(cfg.frac), cfg.r0, cfg.L0, osys.model, i) for i in range(osys.N)]
+        with ProcessPoolExecutor(max_workers=min(osys.N, cores)) as ex:
+            osys.theta = sum(ex.map(_oracle_generator_rows, jobs))
+        s = np.asarray(screens.generate(cfg, osys.sigma2)["slopes"][0].ravel(), dtype=np.float64)
+
+        def step():
+            t0 = time.perf_counter()
+            x, _ = osys.solve_cg(s, n_iter)
+            for t in range(len(cfg.targets)):
+                osys.reconstruct(x, t)
+            return time.perf_counter() - t0
+        return step, (f"matrix-free fp64 oracle, whole step: {n_iter} direct-sum Sigma_ss products (oracle/directsum.c, OpenMP) in the "
+                      f"oracle's CG + the matrix-free projection to {len(cfg.targets)} target(s)"), cores, False
     # the direct sum's cost does not depend on the generator values: only the rows of WFS 0 are built (the oracle's
     # numpy generator build takes minutes for all N^2 pairs); the product itself is timed in full
     theta = tz.css_generators(cfg.n, cfg.d, osys.dirs, osys.h_gs, cfg.h, cfg.frac, cfg.r0, cfg.L0, wfs_rows=[0])
@@ -127,35 +152,85 @@ def oracle_setup(cfg, n_iter):
     directsum.css_mvm(theta, osys.ix, osys.iy, v)
 
     def step():
-        t0 = time.perf_counter()
-        directsum.css_mvm(theta, osys.ix, osys.iy, v)
-        return (time.perf_counter() - t0) * n_iter
-    return step, (f"matrix-free fp64 oracle (oracle/directsum.c, OpenMP): one full direct-sum Sigma_ss product timed, "
-                  f"x{n_iter} iterations; target projection not included"), cores
+        ts = []
+        for _ in range(5):
+            t0 = time.perf_counter()
+            directsum.css_mvm(theta, osys.ix, osys.iy, v)
+            ts.append(time.perf_counter() - t0)
+        return statistics.median(ts) * n_iter
+    return step, (f"matrix-free fp64 oracle (oracle/directsum.c, OpenMP): median of 5 timed direct-sum Sigma_ss products "
+                  f"x {n_iter} iterations (extrapolated; target projection not included)"), cores, True
+
+
+def workload_config(cfg, plan_P, plan_P_os, n_iter, batch, solver, method, world):
+    return {"workload": cfg.name, "n": cfg.n, "n_wfs": cfg.n_wfs, "n_layers": cfg.n_layers, "pad": plan_P, "pad_os": plan_P_os,
+            "n_iter": n_iter, "batch": batch, "targets": len(cfg.targets), "solver": solver, "method": method,
+            "parallelism": f"replicas x{world}", "l2": "flushed (256 MiB write) before every timed step"}
 
 
 def run_reference(args, cfg, n_iter, rank):
     if rank != 0:
         return
-    step, desc, cores = oracle_setup(cfg, n_iter)
-    for _ in range(min(max(args.warmup, 0), 2)):
+    from paper_1806_07938_b200 import tomo
+    step, desc, cores, extrapolated = oracle_setup(cfg, n_iter, whole=True)
+    elt = 2 * cfg.n_wfs * cfg.n * cfg.n > 6000
+    w = 0 if elt else min(max(args.warmup, 0), 2)           # a whole ELT step takes the oracle around half a minute
+    for _ in range(w):
         step()
-    k = max(1, min(args.steps, 5))
+    k = max(1, min(args.steps, 1 if elt else 5))
     sec = statistics.mean(step() for _ in range(k))
     val = 1.0 / sec
+    sz = tomo.host_sizes(cfg, cfg.pad, cfg.pad_os)
+    config = workload_config(cfg, sz["P"], sz["P_os"], n_iter, 1, "oracle (fp64, host cores)", "cg", 1)
+    config["l2"] = "n/a (host)"
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": "reconstructions/s", "n_gpus": args.gpus,
-            "steps": k, "warmup": min(max(args.warmup, 0), 2), "ms_per_step": sec * 1e3, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": cfg.name, "batch": 1, "n_iter": n_iter},
-            "us_per_cg_iteration": sec / n_iter * 1e6,
+            "steps": k, "warmup": w, "ms_per_step": sec * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config,
+            "us_per_cg_iteration": sec / n_iter * 1e6, "extrapolated": extrapolated,
             "cpu_baseline": {"value": val, "unit": "reconstructions/s", "cores": cores, "kind": "oracle", "sample": desc},
             "e2e": {"value": val, "unit": "reconstructions/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line))
 
 
 # ------------------------------------------------------------------------------------------------ our arm
+def respawn_under_torchrun(args):
+    """`python bench.py --gpus N` with no rendezvous in the environment: start the N ranks ourselves (one process per GPU,
+    torch.distributed.run on 127.0.0.1) and let rank 0 print the line."""
+    import socket
+    import subprocess
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd))
+
+
+def kernel_source_hash():
+    """sha256 (16 hex digits) of the persistent kernel's sources: ties a stored ncu traffic figure to the code it was taken from."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in ("persist_kernel.cuh", "persist_host.cuh", "solve_persistent.cu", "fft_reg.cuh"):
+        h.update(open(os.path.join(ROOT, "paper_1806_07938_b200", "csrc", f), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def stored_traffic(workload, batch, precision):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one k_persistent launch from the committed ncu capture
+    (profiles/r2_traffic.json), or None when there is none for this (workload, batch, precision) or the kernel has changed since."""
+    p = os.path.join(ROOT, "profiles", "r2_traffic.json")
+    if not os.path.exists(p):
+        return None
+    for e in json.load(open(p)).get("entries", []):
+        if (e["workload"], e["batch"], e["precision"]) == (workload, batch, precision) and e["kernel_source_hash"] == kernel_source_hash():
+            return e["dram_bytes_per_launch"]
+    return None
+
+
 def main():
     args = parse()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        respawn_under_torchrun(args)
     from tomo_inputs.configs import get_config
     cfg = get_config(args.config)
     n_iter = args.n_iter or cfg.n_iter
@@ -179,8 +254,6 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     prec = {"f32": tomo.TOMO_F32, "f32s_f64a": tomo.TOMO_F32S_F64A, "f64": tomo.TOMO_F64}[args.precision]
-    if args.method == "minres":
-        args.solver = "multikernel"          # tomo_solve_minres runs on the multi-kernel path
     solver = tomo.TOMO_SOLVER_PERSISTENT if args.solver == "persistent" else tomo.TOMO_SOLVER_MULTIKERNEL
     B = args.batch
     t0 = time.perf_counter()
@@ -282,15 +355,14 @@ def main():
     if args.solver == "persistent":
         # the dominant kernel is the persistent solver itself: device time of the launch alone (CUDA events on the stream)
         reps = max(3, min(args.steps, 50))
-        k_ms = plan.time_solver(d_slopes, B, n_iter, reps, stream=stream)
-        k_ms0 = plan.time_solver(d_slopes, B, 0, reps, stream=stream)
+        k_ms = plan.time_solver(d_slopes, B, n_iter, reps, stream=stream, minres=minres)
+        k_ms0 = plan.time_solver(d_slopes, B, 0, reps, stream=stream, minres=minres)
         kb = n_iter * b_iter + B * 4 * Ns * E
         ach = kb / (k_ms * 1e-3) / 1e9
         roof = {"kernel": "k_persistent", "bound": "hbm", "achieved": ach, "peak": hbm, "unit": "GB/s", "frac": ach / hbm,
-                # dram__bytes_read.sum + dram__bytes_write.sum of one launch, ncu --set full (profiles/r1_persistent_ncu_details.md:
-                # 8.550 MB + 0.133 MB at batch 1, 11.71 MB + 36.45 MB at batch 16)
-                "traffic": 8683264 if (cfg.name.startswith("cfg3") and B == 1 and args.precision == "f32") else
-                           (48158976 if (cfg.name.startswith("cfg3") and B == 16 and args.precision == "f32") else None),
+                # dram__bytes_read.sum + dram__bytes_write.sum of one launch from the committed ncu capture of THIS kernel source
+                # (profiles/r2_traffic.json, keyed by workload, batch, precision and source hash), else null
+                "traffic": stored_traffic(cfg.name, B, args.precision), "kernel_source_hash": kernel_source_hash(),
                 "peak_source": how, "algorithmic_bytes_per_launch": kb,
                 "ms_per_launch": k_ms, "ms_per_launch_n_iter0": k_ms0,
                 "us_per_iteration_in_kernel": (k_ms - k_ms0) / n_iter * 1e3,
@@ -323,10 +395,7 @@ def main():
     line = {"metric": METRIC, "value": value, "unit": "reconstructions/s", "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": args.precision, "data": "synthetic",
-            "config": {"workload": cfg.name, "n": cfg.n, "n_wfs": cfg.n_wfs, "n_layers": cfg.n_layers, "pad": plan.P,
-                       "pad_os": plan.P_os, "n_iter": n_iter, "batch": B, "targets": len(cfg.targets),
-                       "solver": args.solver, "method": args.method, "parallelism": f"replicas x{world}",
-                       "l2": "flushed (256 MiB write) before every timed step"},
+            "config": workload_config(cfg, plan.P, plan.P_os, n_iter, B, args.solver, args.method, world),
             "us_per_cg_iteration": us_iter, "ms_per_step_n_iter0": ms_step0, "ms_per_step_l2_warm": ms_step_warm,
             "reconstructions_per_s_l2_warm": world * B * 1e3 / ms_step_warm,
             "iteration_roofline": iter_roof, "l2_roofline": l2_roof, "roofline": roof,
@@ -335,10 +404,10 @@ def main():
             "gpu_launches": launches * args.steps, "launches_per_step": launches, "clocks": clocks,
             "plan_build_s": t_plan, "device_bytes": plan.stats()["device_bytes"]}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        step, desc, cores = oracle_setup(cfg, n_iter)
-        sec = statistics.mean(step() for _ in range(3))
+        step, desc, cores, extrapolated = oracle_setup(cfg, n_iter, whole=False)
+        sec = statistics.median(step() for _ in range(3))
         line["cpu_baseline"] = {"value": 1.0 / sec, "unit": "reconstructions/s", "cores": cores, "kind": "oracle",
-                                "sample": desc, "us_per_cg_iteration": sec / n_iter * 1e6}
+                                "sample": desc, "extrapolated": extrapolated, "us_per_cg_iteration": sec / n_iter * 1e6}
     if rank == 0:
         print(json.dumps(line))
     plan.close()

@@ -130,7 +130,9 @@ int tomo_solve_batch(tomo_plan *plan, const float *slopes, float *wavefront_out,
  * Sigma_ss product kernels, exactly n_iter iterations, no preconditioner, then the projection to every target.
  * Arguments, layouts, ownership and errors as tomo_solve_batch (x0 = optional warm start, NULL = cold start).
  * tomo_get_residuals afterwards returns phibar_k = |b - A x_k|, k = 0..n_iter; tomo_get_zeta the iterate x_{n_iter}.
- * Runs on the multi-kernel solver (one CUDA graph per solve) whatever the plan's `solver` option is. */
+ * Runs on the solver that runs the plan (tomo_get_solver): inside the persistent kernel -- the same two phases and two grid
+ * exchanges per iteration as CG, alpha_k = v_k . A v_k by Parseval where CG takes p.q, beta_{k+1} = |u_k| where CG takes r.r --
+ * or as one CUDA graph of the multi-kernel solver. */
 int tomo_solve_minres(tomo_plan *plan, const float *slopes, float *wavefront_out, int n_frames, int n_iter,
                       const float *x0, void *cuda_stream);
 
@@ -168,10 +170,10 @@ int tomo_time_kernels(tomo_plan *plan, int n_frames, int n_iter, float *ms_out, 
 int tomo_time_phases(tomo_plan *plan, int n_frames, int n_iter, float *us_out, void *cuda_stream);
 
 /* Measurement aid (bench.py "roofline" with the persistent solver): `reps` launches of the persistent kernel alone
- * (A1-A6: rhs projection + n_iter CG iterations from a cold start on `slopes`, device fp32 [n_frames][C][n_vs]; no
+ * (A1-A6: rhs projection + n_iter CG (minres = 0) or MINRES (minres != 0) iterations from a cold start on `slopes`, device fp32 [n_frames][C][n_vs]; no
  * target projection), each bracketed by CUDA events on `cuda_stream`; synchronises the stream and returns the mean
  * device time of one launch in ms (host fp32 [1]). */
-int tomo_time_solver(tomo_plan *plan, const float *slopes, int n_frames, int n_iter, int reps, float *ms_out,
+int tomo_time_solver(tomo_plan *plan, const float *slopes, int n_frames, int n_iter, int reps, int minres, float *ms_out,
                      void *cuda_stream);
 
 /* Measurement aid (bench.py "l2_roofline", north_star: "... and over L2 bandwidth where the spectra are L2-resident"): the

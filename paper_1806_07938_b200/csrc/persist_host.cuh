@@ -3,6 +3,7 @@
 #pragma once
 #include <algorithm>
 #include <cstring>
+#include <set>
 #include <string>
 #include <type_traits>
 #include <vector>
@@ -19,13 +20,13 @@ namespace tomo {
 struct PersistState {
     unsigned *d_flags = nullptr;
     void *d_T1 = nullptr, *d_T1p = nullptr, *d_T2 = nullptr, *d_mspec = nullptr, *d_s2c = nullptr;
-    void *d_xd = nullptr, *d_rd = nullptr, *d_pd = nullptr, *d_bd = nullptr;
+    void *d_xd = nullptr, *d_rd = nullptr, *d_pd = nullptr, *d_bd = nullptr, *d_w1d = nullptr, *d_w2d = nullptr;
     double *d_part_r = nullptr, *d_part_s = nullptr, *d_part_i = nullptr;
-    int G = 0, nq_m = 1, NQ = 0, SB = 0, any_remove = 0, spec_smem = 0, vec_smem = 0;
+    int G = 0, nq_m = 1, NQ = 0, NQ_mr = 0, SB = 0, any_remove = 0, spec_smem = 0, vec_smem = 0, vec_smem_mr = 0;
     int off_ms = 0, off_work = 0, off_red = 0, off_scal = 0, off_tab = 0, off_upart = 0, off_vm = 0, off_vec = 0, off_spec = 0, off_ptab = 0, off_unit = 0, ngs = 2;
     int off_ms2 = 0, fb = 1;
     size_t smem = 0;
-    bool attr_set = false, attr_set_batch = false, attr_set_prof = false, attr_set_prof_batch = false;
+    std::set<const void *> attr_set;    // kernel instances whose dynamic shared-memory limit has been raised
     int *d_seg = nullptr;        // [F_max + 1][sms][8] slab segment tables, one per frame count (slab_segments), uploaded by persist_prepare
     int sms = 0;
 };
@@ -34,7 +35,7 @@ struct PersistState {
 void slab_segments(int Ph, int F, int G, std::vector<int> &seg);
 
 struct PLaunch {
-    int F, n_iter, mode, finalize_p;
+    int F, n_iter, mode, finalize_p, method;
     const float *slopes, *x0;
     double *scal_out;
     long long *dbg;
@@ -79,20 +80,23 @@ static int persist_launch(tomo_plan *pl, cudaStream_t st, const PLaunch &L) {
     a.part_r = ps->d_part_r; a.part_s = ps->d_part_s; a.part_i = ps->d_part_i;
     a.hist = pl->d_hist; a.hist_stride = pl->hist_cap; a.alpha = pl->d_alpha; a.scal_out = L.scal_out;
     a.flags = ps->d_flags; a.dbg = L.dbg;
-    // the instrumented instances (tomo_time_phases) exist for TOMO_F32 only; the production instances carry no stamp code
-    const void *kern = L.F > 1 ? (const void *)(k_persistent<T, S, P, true, false>) : (const void *)(k_persistent<T, S, P, false, false>);
+    // the instrumented instances (tomo_time_phases) exist for TOMO_F32 and CG only; the production instances carry no stamp code
+    const bool mr = L.method == METHOD_MINRES;
+    const void *kern = mr ? (L.F > 1 ? (const void *)(k_persistent<T, S, P, true, false, METHOD_MINRES>) : (const void *)(k_persistent<T, S, P, false, false, METHOD_MINRES>))
+                          : (L.F > 1 ? (const void *)(k_persistent<T, S, P, true, false, METHOD_CG>) : (const void *)(k_persistent<T, S, P, false, false, METHOD_CG>));
     if (L.dbg) {
-        if constexpr (std::is_same<T, float>::value && std::is_same<S, float>::value)
-            kern = L.F > 1 ? (const void *)(k_persistent<T, S, P, true, true>) : (const void *)(k_persistent<T, S, P, false, true>);
-        else { set_error("tomo_time_phases: the instrumented kernel instances exist for TOMO_F32 only"); return TOMO_EUNSUPPORTED; }
+        if constexpr (std::is_same<T, float>::value && std::is_same<S, float>::value) {
+            if (mr) { set_error("tomo_time_phases: the instrumented kernel instances run CG"); return TOMO_EUNSUPPORTED; }
+            kern = L.F > 1 ? (const void *)(k_persistent<T, S, P, true, true, METHOD_CG>) : (const void *)(k_persistent<T, S, P, false, true, METHOD_CG>);
+        } else { set_error("tomo_time_phases: the instrumented kernel instances exist for TOMO_F32 only"); return TOMO_EUNSUPPORTED; }
     }
-    bool &attr_set = L.dbg ? (L.F > 1 ? ps->attr_set_prof_batch : ps->attr_set_prof) : (L.F > 1 ? ps->attr_set_batch : ps->attr_set);
-    if (!attr_set) {
+    if (mr) { a.NQ = ps->NQ_mr; a.vec_smem = ps->vec_smem_mr; a.w1d = (T *)ps->d_w1d; a.w2d = (T *)ps->d_w2d; }
+    if (!ps->attr_set.count(kern)) {
         PCK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ps->smem));
         int occ = 0;
         PCK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kPThreads, ps->smem));
         if (occ < 1) { set_error("persistent kernel does not fit on an SM"); return TOMO_EUNSUPPORTED; }
-        attr_set = true;
+        ps->attr_set.insert(kern);
     }
     PCK(cudaMemsetAsync(ps->d_flags, 0, 1024, st));
     void *kargs[] = {&a};

@@ -45,6 +45,11 @@ enum { PT_START = 0, PT_RHO = 1, PT_BUILD = 2, PT_FFT = 3, PT_MAC = 4, PT_INV = 
 
 // per-frame scalar block in shared memory (doubles)
 enum { SC_RHO = 0, SC_RHO_PREV = 1, SC_BETA = 2, SC_ALPHA = 3, SC_UPD = 4, SC_PQ = 5, SC_HEAD = 6 };
+// ... followed by the 2C channel sums of q, the 3N mode coefficients, and (MINRES) the 2C channel sums of v_k and the state of
+// the Paige-Saunders recurrences at offset SC_HEAD + 4C + 3N:
+enum { MR_C = 0, MR_S = 1, MR_DBAR = 2, MR_EPS = 3, MR_PHIBAR = 4, MR_FROZEN = 5, MR_BETA = 6, MR_INVBETA = 7,
+       MR_PON = 8, MR_PEPS = 9, MR_PDELTA = 10, MR_PINVG = 11, MR_PPHI = 12, MR_N = 16 };
+enum { METHOD_CG = 0, METHOD_MINRES = 1 };
 
 template <typename T, typename S> struct PArgs {
     DevGeom g;
@@ -70,6 +75,7 @@ template <typename T, typename S> struct PArgs {
     const float *x0;             // [F][C][nv] warm start (WARM)
     T *x, *r, *p;                // [F][C][nv] valid-only layout (ABI side)
     T *xd, *rd, *pd, *bd;        // [F][C][npad][n] dense rows (solver side; xd/rd/pd unused with vec_smem)
+    T *w1d, *w2d;                // MINRES: dense rows of w_{k-1}, w_{k-2} (unused with vec_smem)
     typename cx_of<T>::type *T1;    // [F][Ph][C][npad]     x-FFT of the current residual rows
     typename cx_of<T>::type *T1p;   // [F][Ph][C][npad]     x-FFT of the search direction (slab-private state)
     typename cx_of<T>::type *T2;    // [F][C][npairs][Ph][2]
@@ -222,7 +228,7 @@ __device__ __forceinline__ void mac_dispatch(int grp, const typename cx_of<T>::t
 // X: forward y-spectra [c][LD] in natural k_y order; Y: [c][LD], CONJUGATED (the inverse transform is run as a forward
 // one).  CT > 0: the C inputs of this k_y are held in registers; CT = 0: run-time channel count.
 // red: [Goc][P] partial p.q, then [C][P] mask sums, then [C][P] focus sums.
-template <typename T, typename S, int CT, int PP>
+template <typename T, typename S, int CT, int PP, bool MR>
 __device__ __forceinline__ void mac_slab(const typename cx_of<T>::type *X, typename cx_of<T>::type *Y, int LD,
                                          const typename cx_of<S>::type *spec, const PairRef *ptab,
                                          const typename cx_of<T>::type *ms, const T *s2c,
@@ -270,6 +276,15 @@ __device__ __forceinline__ void mac_slab(const typename cx_of<T>::type *X, typen
         }
     }
     red[grp * P + ky] = pap;
+    if (MR && any_remove) {        // MINRES: the same modal sums of the product's INPUT v~ (every v_k is re-projected, reading G27)
+        T *red_v = red_s + (nq_m > 1 ? 2 : 1) * C * P;
+        const T ip2 = (T)1 / ((T)P * (T)P);           // v~ is an unnormalised transform (y~ carries the 1/P^2 folded into the kernel spectra)
+        for (int oc = oc_lo; oc < oc_hi; ++oc) {
+            const C2 xo = X[oc * LD + ky];
+            red_v[oc * P + ky] = ip2 * (m0.x * xo.x + m0.y * xo.y);
+            if (nq_m > 1) { const C2 mm = (oc & 1) ? m2 : m1; red_v[(C + oc) * P + ky] = ip2 * (mm.x * xo.x + mm.y * xo.y); }
+        }
+    }
 }
 
 // fixed-order sum of `cnt` values of the slab partial array by one warp
@@ -282,7 +297,12 @@ template <typename T> __device__ __forceinline__ double warp_sum_red(const T *sr
 // BATCH = false: the single-frame instance (latency-bound: compact code, the CTA's own slab only);
 // BATCH = true: several frames per solve (throughput: balanced slab passes, every global load of a step issued up front).
 // PROF = true: thread 0 stamps clock64 at the phase boundaries (tomo_time_phases); the production instances carry no stamp code.
-template <typename T, typename S, int P, bool BATCH, bool PROF>
+// METHOD_MINRES: the Paige-Saunders recurrences (the solver the paper keeps for the Toeplitz method, S2.G L337, L426; written
+// out in oracle/solver.py:minres, reading G27) in the SAME two phases: the product's input is v_k = u_{k-1} / beta_k (the row
+// phase sends the transform of the unnormalised u, phase C scales it: the transform is linear), alpha_k = v_k . M_s A v_k by
+// Parseval where CG takes p.q, beta_{k+1} = |u_k| where CG takes r.r; the Givens rotation k needs beta_{k+1}, so x_k and w_k are
+// updated one row phase later (the last one in the tail).  Rows of a unit: x, v_{k-1} (CG's r), u_{k-1} (CG's p), w_{k-1}, w_{k-2}.
+template <typename T, typename S, int P, bool BATCH, bool PROF, int METHOD = METHOD_CG>
 __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
     typedef typename cx_of<T>::type C2;
     typedef typename cx_of<S>::type S2;
@@ -309,7 +329,10 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
     PairRef *ptab = reinterpret_cast<PairRef *>(smem_raw + a.off_ptab);
     UnitRec *s_unit = reinterpret_cast<UnitRec *>(smem_raw + a.off_unit);
     const int FB = BATCH ? a.fb : 1;                           // frames per slab pass
-    const int red_sz = (min(kPWarps / ((P + 31) >> 5), C) + 2 * C) * P;      // partial sums of one frame (mac_slab)
+    constexpr bool MINRES = METHOD == METHOD_MINRES;
+    constexpr int NVEC = MINRES ? 5 : 3;                                      // row vectors per unit in shared memory
+    const int red_sz = (min(kPWarps / ((P + 31) >> 5), C) + (MINRES ? 4 : 2) * C) * P;      // partial sums of one frame (mac_slab)
+    const int SCM = SC_HEAD + 2 * C + 3 * N, MRS = SCM + 2 * C;               // MINRES: channel sums of v, recurrence state
     C2 *Ubuf = work, *Vbuf = work + (size_t)FB * C * LD;      // [frame of the pass][c][LD] each
     const int NGS = a.ngs;
     C2 *bufA = work + (size_t)(gs < NGS ? gs : 0) * (P + LD), *bufB = bufA + P;   // row unit: natural [P], pass-1 result [LD]
@@ -402,8 +425,8 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
     };
     // dense rows (2 x n) of x, r, p, b of unit i
     auto dense = [&](int i, const Unit &q, int which) -> T * {
-        if (a.vec_smem && which < 3) return svec + ((size_t)i * 3 + which) * 2 * n;
-        T *base = which == 0 ? a.xd : which == 1 ? a.rd : which == 2 ? a.pd : a.bd;
+        if (a.vec_smem && which != 3) return svec + ((size_t)i * NVEC + (which < 3 ? which : which - 1)) * 2 * n;     // 4, 5: w_{k-1}, w_{k-2}
+        T *base = which == 0 ? a.xd : which == 1 ? a.rd : which == 2 ? a.pd : which == 3 ? a.bd : which == 4 ? a.w1d : a.w2d;
         return base + (((size_t)q.f * C + q.c) * npad + q.y0) * n;
     };
 
@@ -477,6 +500,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
         __syncwarp();
         if (act) {
             for (int e = gl; e < 2 * n; e += kGS) { ux[e] = (T)0; ur[e] = (T)0; up[e] = (T)0; if (a.mode == PM_WARM) ub[e] = (T)0; }
+            if (MINRES) { T *w1 = dense(i, q, 4), *w2 = dense(i, q, 5); for (int e = gl; e < 2 * n; e += kGS) { w1[e] = (T)0; w2[e] = (T)0; } }
             for (int e = gl; e < n; e += kGS) bufA[e] = mk<T>((T)0, (T)0);
         }
         __syncwarp();
@@ -502,6 +526,56 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
     }
     GRID_SYNC();
 
+    // MINRES: what one lane does per frame once |u_{kk-1}|^2 = uu is summed (kk = 0: |r0|^2): rotation kk-1 of the Lanczos
+    // tridiagonal (oracle/solver.py:minres, same order), the coefficients of the pending x / w update, beta_kk for the product's
+    // input, phibar^2 into the history.  Breakdowns freeze the iterate (reading G16 / G27).
+    auto minres_scalars = [&](int f, int kk, double uu) {
+        double *sc = scal + f * SB, *st = sc + MRS;
+        if (kk == 0) {
+            const double beta = sqrt(uu);
+            st[MR_C] = -1.0; st[MR_S] = 0.0; st[MR_DBAR] = 0.0; st[MR_EPS] = 0.0; st[MR_PHIBAR] = beta;
+            st[MR_FROZEN] = beta > 0.0 ? 0.0 : 1.0;
+            st[MR_BETA] = beta; st[MR_INVBETA] = beta > 0.0 ? 1.0 / beta : 0.0; st[MR_PON] = 0.0;
+            if (b == 0) a.hist[(size_t)f * a.hist_stride] = uu;
+            return;
+        }
+        st[MR_PON] = 0.0;
+        if (st[MR_FROZEN] == 0.0) {
+            const double alpha = sc[SC_ALPHA], c = st[MR_C], s_ = st[MR_S], dbar = st[MR_DBAR], phibar = st[MR_PHIBAR];
+            const double beta_next = sqrt(uu);
+            const double delta = c * dbar + s_ * alpha, gbar = s_ * dbar - c * alpha;
+            const double gamma = sqrt(gbar * gbar + beta_next * beta_next);
+            if (!(gamma > 0.0)) {
+                st[MR_FROZEN] = 1.0; st[MR_INVBETA] = 0.0;
+            } else {
+                const double c_new = gbar / gamma, s_new = beta_next / gamma;
+                st[MR_PON] = 1.0; st[MR_PEPS] = st[MR_EPS]; st[MR_PDELTA] = delta; st[MR_PINVG] = 1.0 / gamma; st[MR_PPHI] = c_new * phibar;
+                st[MR_PHIBAR] = s_new * phibar;
+                st[MR_EPS] = s_ * beta_next; st[MR_DBAR] = -c * beta_next; st[MR_C] = c_new; st[MR_S] = s_new;
+                st[MR_BETA] = beta_next;
+                if (beta_next > 0.0) st[MR_INVBETA] = 1.0 / beta_next;
+                else { st[MR_FROZEN] = 1.0; st[MR_INVBETA] = 0.0; }
+            }
+        }
+        if (b == 0) a.hist[(size_t)f * a.hist_stride + kk] = st[MR_PHIBAR] * st[MR_PHIBAR];
+    };
+
+    // MINRES: alpha_k = v_k . M_s q = v.q - (Z^T v)^T (Z^T Z)^-1 Z^T q from the Parseval sums of one frame
+    auto minres_alpha = [&](const double *sc) {
+        double al = sc[SC_PQ];
+        const double *S0 = sc + SC_HEAD, *S1 = S0 + C, *V0 = sc + SCM, *V1 = V0 + C;
+        for (int i = 0; i < N; ++i) {
+            const int nr = s_nrem[i];
+            const double tq[3] = {S0[2 * i], S0[2 * i + 1], S1[2 * i] + S1[2 * i + 1]}, tp[3] = {V0[2 * i], V0[2 * i + 1], V1[2 * i] + V1[2 * i + 1]};
+            for (int u = 0; u < nr; ++u) {
+                double sq = 0.0;
+                for (int v = 0; v < nr; ++v) sq += sGs[i * 9 + u * 3 + v] * tq[v];
+                al -= tp[u] * sq;
+            }
+        }
+        return al;
+    };
+
     // ================================================================ iterations (k = -1 is the warm-start product A x0)
     const int k_begin = (a.mode == PM_WARM) ? -1 : 0;
     const int n_t1 = C * npairs;                        // complex pairs in one T1 slab
@@ -515,7 +589,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
 #pragma unroll 1
     for (k = k_begin; k < a.n_iter; ++k) {
         const bool pre = k < 0;
-        const bool take_new = pre || k == 0;            // p~ = T1 (p_0, or x0 for the warm-start product)
+        const bool take_new = MINRES || pre || k == 0;  // p~ = T1 (p_0, or x0 for the warm-start product; MINRES: always, v_k = u_{k-1} / beta_k)
         PSTAMP(PT_START);
         // ---------------------------------------------------------- phase C: slab (kx, f)
         const int f_lo = BATCH ? s_seg[0] : 0, n_own = BATCH ? s_seg[1] - f_lo : (b < Ph ? 1 : 0), kx2 = BATCH ? s_seg[2] : kx;
@@ -542,14 +616,18 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                 if (k == 0 && a.mode == PM_STATE) rho = a.hist[(size_t)f * a.hist_stride];
                 else rho = warp_sum_units(a.part_r + (size_t)f * U, U, lane);
                 if (lane == 0) {
-                    double *sc = scal + f * SB;
-                    const double rho_prev = sc[SC_RHO];
-                    const bool upd = (k > 0) && (sc[SC_ALPHA] != 0.0) && (rho_prev > 0.0);
-                    sc[SC_RHO_PREV] = rho_prev;
-                    sc[SC_RHO] = rho;
-                    sc[SC_BETA] = upd ? div_as<T>(rho, rho_prev) : 0.0;
-                    sc[SC_UPD] = upd ? 1.0 : 0.0;
-                    if (b == 0) a.hist[(size_t)f * a.hist_stride + k] = rho;
+                    if (MINRES) {
+                        minres_scalars(f, k, rho);
+                    } else {
+                        double *sc = scal + f * SB;
+                        const double rho_prev = sc[SC_RHO];
+                        const bool upd = (k > 0) && (sc[SC_ALPHA] != 0.0) && (rho_prev > 0.0);
+                        sc[SC_RHO_PREV] = rho_prev;
+                        sc[SC_RHO] = rho;
+                        sc[SC_BETA] = upd ? div_as<T>(rho, rho_prev) : 0.0;
+                        sc[SC_UPD] = upd ? 1.0 : 0.0;
+                        if (b == 0) a.hist[(size_t)f * a.hist_stride + k] = rho;
+                    }
                 }
             }
         }
@@ -579,10 +657,12 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                     const int e2 = tid + m * kPThreads;
                     if (e2 < n_t1) {
                         C2 v0, v1;
-                        if (take_new) { v0 = n0[m]; v1 = n1[m]; }
-                        else if (upd) { v0 = mk<T>(n0[m].x + beta * o0[m].x, n0[m].y + beta * o0[m].y); v1 = mk<T>(n1[m].x + beta * o1[m].x, n1[m].y + beta * o1[m].y); }
+                        if (take_new) {
+                            v0 = n0[m]; v1 = n1[m];
+                            if (MINRES && !pre) { const T ib = (T)sc[MRS + MR_INVBETA]; v0.x *= ib; v0.y *= ib; v1.x *= ib; v1.y *= ib; }
+                        } else if (upd) { v0 = mk<T>(n0[m].x + beta * o0[m].x, n0[m].y + beta * o0[m].y); v1 = mk<T>(n1[m].x + beta * o1[m].x, n1[m].y + beta * o1[m].y); }
                         else { v0 = o0[m]; v1 = o1[m]; }
-                        if (take_new || upd) st_pair(t1p + 2 * e2, v0, v1);
+                        if (!MINRES && (take_new || upd)) st_pair(t1p + 2 * e2, v0, v1);
                         Vf[voff[m]] = v0;
                         if (vtwo[m]) Vf[voff[m] + 1] = v1;
                     }
@@ -597,7 +677,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
             if (p2) dft_pass<T, B, false>(Ubuf + c2s * LD + k1s * (B + 1), 1, B, Vbuf + c2s * LD + k1s, A, tw, 0);
             __syncthreads();
             PSTAMP(PT_FFT);
-#define TOMO_MAC(CT_, SP_) mac_slab<T, S, CT_, P>(Vbuf + (size_t)fr * C * LD, Ubuf + (size_t)fr * C * LD, LD, SP_, ptab, msi, s_s2c, C, P, a.nq_m, a.any_remove, red + fr * red_sz, warp, lane)
+#define TOMO_MAC(CT_, SP_) mac_slab<T, S, CT_, P, METHOD == METHOD_MINRES>(Vbuf + (size_t)fr * C * LD, Ubuf + (size_t)fr * C * LD, LD, SP_, ptab, msi, s_s2c, C, P, a.nq_m, a.any_remove, red + fr * red_sz, warp, lane)
 #define TOMO_MAC_SWITCH(SP_)                                                               \
     switch (C) {                                                                           \
         case 4: TOMO_MAC(4, SP_); break;   case 6: TOMO_MAC(6, SP_); break;                \
@@ -688,10 +768,11 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                 // trip per item cost 7.5 us)
                 // items: p.q of every frame (alpha of the frames of the CTA's slab passes), then the modal sums of the frames
                 // of its row units (batch: one or two frames; single frame: item = qq)
-                constexpr int NLD = (Ph + 31) / 32, NB = BATCH ? 4 : 1;
-                const int n_sc = BATCH ? F + fu_n * (NQ - 1) : F * NQ;
+                constexpr int NLD = (Ph + 31) / 32, NB = BATCH ? 4 : MINRES ? 2 : 1;     // (MINRES has 1 + 2C(+2C) items: two per warp in one trip)
+                // (MINRES: alpha_k of EVERY frame needs that frame's modal sums, for the rotation in the next phase C)
+                const int n_sc = (BATCH && !MINRES) ? F + fu_n * (NQ - 1) : F * NQ;
                 auto sc_item = [&](int item, int &f, int &qq) {
-                    if (!BATCH) { f = item / NQ; qq = item - f * NQ; }
+                    if (!BATCH || MINRES) { f = item / NQ; qq = item - f * NQ; }
                     else if (item < F) { f = item; qq = 0; }
                     else { const int r = item - F; f = fu_lo + r / (NQ - 1); qq = 1 + r % (NQ - 1); }
                 };
@@ -717,7 +798,8 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                             if constexpr (NLD == 5) t = ((v[j][0] + v[j][1]) + (v[j][2] + v[j][3])) + v[j][4];     // the order warp_sum_cg160 used
                             else { t = v[j][0]; for (int m = 1; m < NLD; ++m) t += v[j][m]; }
                             const double s = warp_sum(t);
-                            if (lane == 0) scal[f * SB + (qq == 0 ? SC_PQ : SC_HEAD + qq - 1)] = s;
+                            const int nqs = C * (a.nq_m > 1 ? 2 : 1);             // modal sums of q, then (MINRES) of v
+                            if (lane == 0) scal[f * SB + (qq == 0 ? SC_PQ : qq - 1 < nqs ? SC_HEAD + qq - 1 : SCM + qq - 1 - nqs)] = s;
                         }
                     }
                 }
@@ -728,7 +810,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                     for (int f = tid; f < F; f += kPThreads) {
                         double *sc = scal + f * SB;
                         const double rho = sc[SC_RHO], pq = sc[SC_PQ];
-                        const double al = (rho > 0.0 && pq > 0.0) ? div_as<T>(rho, pq) : 0.0;     // breakdown: freeze (reading G16)
+                        const double al = MINRES ? minres_alpha(sc) : (rho > 0.0 && pq > 0.0) ? div_as<T>(rho, pq) : 0.0;     // breakdown: freeze (reading G16)
                         sc[SC_ALPHA] = al;
                         if (b == 0) a.alpha[f] = al;
                     }
@@ -737,6 +819,21 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
             }
             // stage 2: q' = M_s q, CG vector updates, r.r partial, the new residual rows -> bufA -> forward x-FFT -> T1
             double rr = 0.0;
+            double al_mr = 0.0;                      // MINRES: alpha_k of the unit's frame, one WFS term per lane of the group
+            if (MINRES && !pre) {
+                const double *sc = scal + q.f * SB, *S0 = sc + SC_HEAD, *S1 = S0 + C, *V0 = sc + SCM, *V1 = V0 + C;
+                double term = 0.0;
+                for (int i2 = gl; i2 < N; i2 += kGS) {
+                    const int nr = s_nrem[i2];
+                    const double tq[3] = {S0[2 * i2], S0[2 * i2 + 1], S1[2 * i2] + S1[2 * i2 + 1]}, tp[3] = {V0[2 * i2], V0[2 * i2 + 1], V1[2 * i2] + V1[2 * i2 + 1]};
+                    for (int u = 0; u < nr; ++u) {
+                        double sq = 0.0;
+                        for (int v = 0; v < nr; ++v) sq += sGs[i2 * 9 + u * 3 + v] * tq[v];
+                        term += tp[u] * sq;
+                    }
+                }
+                al_mr = sc[SC_PQ] - group_sum(term);
+            }
             if (act) {
                 const double *sc = scal + q.f * SB;
                 const double rho_k = sc[SC_RHO], pq_k = sc[SC_PQ];
@@ -819,8 +916,81 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                         }
                     }
                 };
-                if (a.vec_smem) {
-                    T *base = svec + (size_t)i * 6 * n;
+                // MINRES (one Lanczos step + the x / w update of the PREVIOUS iteration, whose rotation needed |u|): rows x, v_{k-1},
+                // u_{k-1} (v_k = u_{k-1} / beta_k, re-projected: reading G27), w_{k-1}, w_{k-2}
+                auto update_rows_mr = [&](T *ux, T *uvo, T *uvc, T *uw1, T *uw2) {
+                    const double *st = sc + MRS;
+                    const bool frozen = st[MR_FROZEN] != 0.0, first = k == 0, pon = st[MR_PON] != 0.0;
+                    const T alm = (T)al_mr, betak = (T)st[MR_BETA], ib = (T)st[MR_INVBETA];
+                    const T peps = (T)st[MR_PEPS], pdelta = (T)st[MR_PDELTA], pinvg = (T)st[MR_PINVG], pphi = (T)st[MR_PPHI];
+                    T cv0 = (T)0, cv2 = (T)0;                             // mode coefficients of v_k
+                    {
+                        const double *V0 = sc + SCM, *V1 = V0 + C;
+                        const double tp[3] = {V0[2 * q.w], V0[2 * q.w + 1], V1[2 * q.w] + V1[2 * q.w + 1]};
+                        const int nr = s_nrem[q.w];
+                        const double *Gw = sGs + q.w * 9;
+                        double d0 = 0.0, d2 = 0.0;
+                        for (int v = 0; v < nr; ++v) { d0 += Gw[q.comp * 3 + v] * tp[v]; d2 += Gw[6 + v] * tp[v]; }
+                        cv0 = (q.comp < nr) ? (T)d0 : (T)0;
+                        cv2 = (2 < nr) ? (T)d2 : (T)0;
+                    }
+                    constexpr int NX = (P / 2 + kGS) / kGS;              // columns per lane
+                    T vo_[NX][2], vc_[NX][2], w1_[NX][2], w2_[NX][2], xv_[NX][2];        // every load is issued before the first store
+#pragma unroll
+                    for (int m = 0; m < NX; ++m) {
+                        const int xp = gl + m * kGS;
+#pragma unroll
+                        for (int row = 0; row < 2; ++row) {
+                            vo_[m][row] = vc_[m][row] = w1_[m][row] = w2_[m][row] = xv_[m][row] = (T)0;
+                            if (xp < n && ((vm >> (row * 16 + m)) & 1u)) {
+                                const int idx = row * n + xp;
+                                if (!first) vo_[m][row] = uvo[idx];
+                                vc_[m][row] = uvc[idx];
+                                if (pon) { w1_[m][row] = uw1[idx]; w2_[m][row] = uw2[idx]; xv_[m][row] = ux[idx]; }
+                            }
+                        }
+                    }
+#pragma unroll
+                    for (int m = 0; m < NX; ++m) {
+                        const int xp = gl + m * kGS;
+                        if (xp < n) {
+                            const C2 z = bufA[xp];
+                            T nr[2] = {(T)0, (T)0};
+#pragma unroll
+                            for (int row = 0; row < 2; ++row) {
+                                if ((vm >> (row * 16 + m)) & 1u) {
+                                    const int idx = row * n + xp;
+                                    const T coord = ((q.comp ? (T)(q.y0 + row) : (T)xp) - half_n) * dd;
+                                    const T vo = vo_[m][row];
+                                    if (pon) {
+                                        const T w = (vo - peps * w2_[m][row] - pdelta * w1_[m][row]) * pinvg;
+                                        ux[idx] = xv_[m][row] + pphi * w;
+                                        uw2[idx] = w1_[m][row]; uw1[idx] = w;
+                                    }
+                                    if (!frozen) {
+                                        const T vp = vc_[m][row] * ib - (cv0 + cv2 * coord);
+                                        const T qp = (row ? -z.y : z.x) - (c0 + c2 * coord);
+                                        const T uv = qp - alm * vp - betak * vo;
+                                        uvo[idx] = vp; uvc[idx] = uv;
+                                        rr += (double)uv * (double)uv;
+                                        nr[row] = uv;
+                                    }
+                                }
+                            }
+                            bufA[xp] = mk<T>(nr[0], nr[1]);
+                        }
+                    }
+                };
+                if (MINRES && !pre) {
+                    if (a.vec_smem) {
+                        T *base = svec + (size_t)i * NVEC * 2 * n;
+                        update_rows_mr(base, base + 2 * n, base + 4 * n, base + 6 * n, base + 8 * n);
+                    } else {
+                        const size_t o = (((size_t)q.f * C + q.c) * npad + q.y0) * n;
+                        update_rows_mr(a.xd + o, a.rd + o, a.pd + o, a.w1d + o, a.w2d + o);
+                    }
+                } else if (a.vec_smem) {
+                    T *base = svec + (size_t)i * NVEC * 2 * n;
                     update_rows(base, base + 2 * n, base + 4 * n);
                 } else {
                     const size_t o = (((size_t)q.f * C + q.c) * npad + q.y0) * n;
@@ -840,19 +1010,24 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
     k = -2;
 
     // ================================================================ tail: rho_{n_iter}; optional p = r + beta p; x, r, p -> valid-only layout
+    // (MINRES: the last rotation and the pending x update)
     for (int f = NW - 1 - warp; f < F; f += NW) {
         double rho;
         if (a.n_iter == 0 && a.mode == PM_STATE) rho = a.hist[(size_t)f * a.hist_stride];
         else rho = warp_sum_units(a.part_r + (size_t)f * U, U, lane);
         if (lane == 0) {
-            double *sc = scal + f * SB;
-            const double rho_prev = sc[SC_RHO];
-            const bool upd = (a.n_iter > 0) && (sc[SC_ALPHA] != 0.0) && (rho_prev > 0.0);
-            sc[SC_BETA] = upd ? div_as<T>(rho, rho_prev) : 0.0;
-            sc[SC_UPD] = upd ? 1.0 : 0.0;
-            if (b == 0) {
-                a.hist[(size_t)f * a.hist_stride + a.n_iter] = rho;
-                if (a.scal_out && f == 0) { a.scal_out[0] = rho; a.scal_out[1] = sc[SC_ALPHA]; a.scal_out[2] = sc[SC_BETA]; }
+            if (MINRES) {
+                minres_scalars(f, a.n_iter, rho);
+            } else {
+                double *sc = scal + f * SB;
+                const double rho_prev = sc[SC_RHO];
+                const bool upd = (a.n_iter > 0) && (sc[SC_ALPHA] != 0.0) && (rho_prev > 0.0);
+                sc[SC_BETA] = upd ? div_as<T>(rho, rho_prev) : 0.0;
+                sc[SC_UPD] = upd ? 1.0 : 0.0;
+                if (b == 0) {
+                    a.hist[(size_t)f * a.hist_stride + a.n_iter] = rho;
+                    if (a.scal_out && f == 0) { a.scal_out[0] = rho; a.scal_out[1] = sc[SC_ALPHA]; a.scal_out[2] = sc[SC_BETA]; }
+                }
             }
         }
     }
@@ -862,15 +1037,21 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
         if (gs >= NGS || i >= nu) continue;
         const Unit q = unit_of(i);
         const double *sc = scal + q.f * SB;
-        const bool fin = a.finalize_p && sc[SC_UPD] != 0.0;
+        const bool fin = !MINRES && a.finalize_p && sc[SC_UPD] != 0.0;
         const T beta = (T)sc[SC_BETA];
         const T *ux = dense(i, q, 0), *ur = dense(i, q, 1), *up = dense(i, q, 2);
+        const double *st = sc + MRS;
+        const bool pon = MINRES && st[MR_PON] != 0.0;
+        const T peps = pon ? (T)st[MR_PEPS] : (T)0, pdelta = pon ? (T)st[MR_PDELTA] : (T)0, pinvg = pon ? (T)st[MR_PINVG] : (T)0,
+                pphi = pon ? (T)st[MR_PPHI] : (T)0;
+        const T *uw1 = MINRES ? dense(i, q, 4) : ux, *uw2 = MINRES ? dense(i, q, 5) : ux;
         for (int e = q.s0 + gl; e < q.s2; e += kGS) {
             const int row = e >= q.s1, idx = row * n + a.g.ix[e];
-            T pv = up[idx];
+            T pv = up[idx], xv = ux[idx];
             const T rv = ur[idx];
             if (fin) pv = rv + beta * pv;
-            a.x[q.vbase + e] = ux[idx]; a.r[q.vbase + e] = rv; a.p[q.vbase + e] = pv;
+            if (pon) xv += pphi * ((rv - peps * uw2[idx] - pdelta * uw1[idx]) * pinvg);      // x_n = x_{n-1} + phi_n w_n, w_n from v_n = rv
+            a.x[q.vbase + e] = xv; a.r[q.vbase + e] = rv; a.p[q.vbase + e] = pv;
         }
     }
 #undef PSTAMP

@@ -123,7 +123,8 @@ static int persist_prepare(tomo_plan *pl) {
     for (int i = 0; i < m.n_wfs; ++i) { if (m.n_remove[i] > 0) ps->any_remove = 1; if (m.n_remove[i] > 2) focus = true; }
     ps->nq_m = focus ? 3 : 1;
     ps->NQ = 1 + m.C * (focus ? 2 : 1);
-    ps->SB = SC_HEAD + 2 * m.C + 3 * m.n_wfs;
+    ps->NQ_mr = 1 + 2 * m.C * (focus ? 2 : 1);            // MINRES: the modal sums of v_k too (reading G27)
+    ps->SB = SC_HEAD + 4 * m.C + 3 * m.n_wfs + MR_N;       // CG block, then MINRES' sums of v and recurrence state
     const size_t E = pl->elem, SE = pl->selem;
     const int WPG = (m.P + 31) / 32, Goc = std::min(kPWarps / WPG, m.C);
     const int maxu = (F * U + ps->G - 1) / ps->G;
@@ -140,7 +141,7 @@ static int persist_prepare(tomo_plan *pl) {
     ps->off_work = (int)(off = align16(off));
     off += std::max((size_t)2 * ps->fb * m.C * LD, (size_t)ps->ngs * (m.P + LD)) * 2 * E;
     ps->off_red = (int)(off = align16(off));
-    off += (size_t)ps->fb * (Goc + 2 * m.C) * m.P * E;
+    off += (size_t)ps->fb * (Goc + 4 * m.C) * m.P * E;
     ps->off_scal = (int)(off = align16(off));
     off += (size_t)F * ps->SB * sizeof(double);
     ps->off_tab = (int)(off = align16(off));
@@ -154,7 +155,7 @@ static int persist_prepare(tomo_plan *pl) {
     ps->off_unit = (int)(off = align16(off));
     off += (size_t)std::max(maxu, 1) * sizeof(UnitRec);
     off = align16(off);
-    const size_t spec_bytes = (size_t)m.n_pair * m.P * 2 * SE, vec_bytes = (size_t)maxu * 6 * m.n * E;
+    const size_t spec_bytes = (size_t)m.n_pair * m.P * 2 * SE, vec_bytes = (size_t)maxu * 6 * m.n * E, vec_bytes_mr = (size_t)maxu * 10 * m.n * E;
     const char *no_pin = getenv("TOMO_NO_SPEC_SMEM"), *no_vec = getenv("TOMO_NO_VEC_SMEM");
     // the spectra slice has priority for the shared memory that is left, then the CG vectors of the CTA's row units
     ps->off_spec = (int)off;
@@ -162,7 +163,8 @@ static int persist_prepare(tomo_plan *pl) {
     if (ps->spec_smem) off = align16(off + spec_bytes);
     ps->off_vec = (int)off;
     ps->vec_smem = (off + vec_bytes <= (size_t)max_smem) && !(no_vec && no_vec[0] == '1');
-    if (ps->vec_smem) off = align16(off + vec_bytes);
+    ps->vec_smem_mr = ps->vec_smem && (off + vec_bytes_mr <= (size_t)max_smem);      // MINRES keeps five row vectors per unit
+    if (ps->vec_smem) off = align16(off + (ps->vec_smem_mr ? vec_bytes_mr : vec_bytes));
     if (off > (size_t)max_smem) { delete ps; set_error("persistent solver: problem too large for shared memory"); return TOMO_EUNSUPPORTED; }
     ps->smem = off;
 
@@ -191,7 +193,8 @@ static int persist_prepare(tomo_plan *pl) {
     PTRY(palloc(pl, &ps->d_pd, dsz));
     PTRY(palloc(pl, &ps->d_bd, dsz));
     PTRY(palloc(pl, (void **)&ps->d_part_r, (size_t)F * U * sizeof(double)));
-    PTRY(palloc(pl, (void **)&ps->d_part_s, (size_t)F * m.Ph * ps->NQ * sizeof(double)));
+    PTRY(palloc(pl, (void **)&ps->d_part_s, (size_t)F * m.Ph * ps->NQ_mr * sizeof(double)));
+    if (!ps->vec_smem_mr) { PTRY(palloc(pl, &ps->d_w1d, dsz)); PTRY(palloc(pl, &ps->d_w2d, dsz)); }
     PTRY(palloc(pl, (void **)&ps->d_part_i, (size_t)F * U * 2 * sizeof(double)));
     PTRY(palloc(pl, &ps->d_mspec, (size_t)ps->nq_m * m.Ph * m.P * 2 * E));
     PTRY(palloc(pl, &ps->d_s2c, (size_t)m.C * E));
@@ -214,9 +217,10 @@ static int persist_prepare(tomo_plan *pl) {
 }
 
 static int persist_dispatch(tomo_plan *pl, cudaStream_t st, int F, int n_iter, int mode, int finalize_p, const float *slopes,
-                            const float *x0, double *scal_out, long long *dbg = nullptr) {
+                            const float *x0, double *scal_out, long long *dbg = nullptr, int method = METHOD_CG) {
     PLaunch L;
     L.F = F; L.n_iter = n_iter; L.mode = mode; L.finalize_p = finalize_p; L.slopes = slopes; L.x0 = x0; L.scal_out = scal_out; L.dbg = dbg;
+    L.method = method;
     switch (pl->m.P) {
 #define TOMO_PCASE(P_) case P_: return persist_run<P_>(pl, st, L);
         TOMO_PERSIST_SIZES(TOMO_PCASE)
@@ -236,6 +240,21 @@ int solve_persistent(tomo_plan *pl, const float *slopes, float *out, int F, int 
     if ((rc = persist_prepare(pl))) return rc;
     pl->launches_last = 0;
     if ((rc = persist_dispatch(pl, st, F, n_iter, x0 ? PM_WARM : PM_COLD, 0, slopes, x0, nullptr))) return rc;
+    if (pl->has_cos && out) {
+        if ((rc = project_from_x(pl, st, F))) return rc;
+        PCK(cudaMemcpyAsync(out, pl->d_out, (size_t)F * pl->m.T * pl->m.nvp * sizeof(float), cudaMemcpyDeviceToDevice, st));
+    }
+    pl->last_frames = F; pl->last_iter = n_iter;
+    return TOMO_OK;
+}
+
+// MINRES (the paper's solver for the Toeplitz method, L337, L426) inside the persistent kernel: same phases, same two exchanges
+// per iteration as CG (persist_kernel.cuh: METHOD_MINRES)
+int solve_minres_persistent(tomo_plan *pl, const float *slopes, float *out, int F, int n_iter, const float *x0, cudaStream_t st) {
+    int rc;
+    if ((rc = persist_prepare(pl))) return rc;
+    pl->launches_last = 0;
+    if ((rc = persist_dispatch(pl, st, F, n_iter, x0 ? PM_WARM : PM_COLD, 0, slopes, x0, nullptr, nullptr, METHOD_MINRES))) return rc;
     if (pl->has_cos && out) {
         if ((rc = project_from_x(pl, st, F))) return rc;
         PCK(cudaMemcpyAsync(out, pl->d_out, (size_t)F * pl->m.T * pl->m.nvp * sizeof(float), cudaMemcpyDeviceToDevice, st));
@@ -331,7 +350,7 @@ int time_phases_persistent(tomo_plan *pl, int F, int n_iter, float *us_out, cuda
 }
 
 // Measurement aid (tomo_time_solver): the persistent kernel alone, `reps` cold-start launches bracketed by events.
-int time_solver_persistent(tomo_plan *pl, const float *slopes, int F, int n_iter, int reps, float *ms_out, cudaStream_t st) {
+int time_solver_persistent(tomo_plan *pl, const float *slopes, int F, int n_iter, int reps, int minres, float *ms_out, cudaStream_t st) {
     int rc;
     if ((rc = persist_prepare(pl))) return rc;
     std::vector<cudaEvent_t> ev(2 * (size_t)reps);
@@ -340,7 +359,7 @@ int time_solver_persistent(tomo_plan *pl, const float *slopes, int F, int n_iter
         PersistState *ps = (PersistState *)pl->persist;
         PCK(cudaMemsetAsync(ps->d_flags, 0, 1024, st));     // (the launch below repeats it; keeps the bracket tight)
         PCK(cudaEventRecord(ev[2 * i], st));
-        rc = persist_dispatch(pl, st, F, n_iter, PM_COLD, 0, slopes, nullptr, nullptr);
+        rc = persist_dispatch(pl, st, F, n_iter, PM_COLD, 0, slopes, nullptr, nullptr, nullptr, minres ? METHOD_MINRES : METHOD_CG);
         PCK(cudaEventRecord(ev[2 * i + 1], st));
     }
     cudaError_t e = cudaStreamSynchronize(st);

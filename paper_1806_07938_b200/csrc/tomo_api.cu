@@ -750,7 +750,7 @@ namespace tomo {
 int solve_persistent(tomo_plan *pl, const float *slopes, float *out, int F, int n_iter, const float *x0, cudaStream_t st);
 int cg_step_persistent(tomo_plan *pl, float *x, float *r, float *p, double *scal, cudaStream_t st);
 int time_phases_persistent(tomo_plan *pl, int F, int n_iter, float *us_out, cudaStream_t st);
-int time_solver_persistent(tomo_plan *pl, const float *slopes, int F, int n_iter, int reps, float *ms_out, cudaStream_t st);
+int time_solver_persistent(tomo_plan *pl, const float *slopes, int F, int n_iter, int reps, int minres, float *ms_out, cudaStream_t st);
 
 // A7-A8 from the CG solution held in d_x -> d_out (used by the persistent solver)
 int project_from_x(tomo_plan *pl, cudaStream_t st, int F) { return DISPATCH(pl, project_from_x(pl, st, F)); }
@@ -761,6 +761,7 @@ int state_load(tomo_plan *pl, cudaStream_t st, const float *x, const float *r, c
 int state_store(tomo_plan *pl, cudaStream_t st, float *x, float *r, float *p) { return DISPATCH(pl, state_store(pl, st, x, r, p)); }
 int vec_store(tomo_plan *pl, cudaStream_t st, const void *src, float *dst) { return DISPATCH(pl, vec_store(pl, st, src, dst)); }
 int apply_css_persistent(tomo_plan *pl, const float *v, float *out, cudaStream_t st);
+int solve_minres_persistent(tomo_plan *pl, const float *slopes, float *out, int F, int n_iter, const float *x0, cudaStream_t st);
 }  // namespace tomo
 
 extern "C" int tomo_solve_batch(tomo_plan *pl, const float *slopes, float *wavefront_out, int n_frames, int n_iter,
@@ -784,6 +785,7 @@ extern "C" int tomo_solve_minres(tomo_plan *pl, const float *slopes, float *wave
     if (n_frames < 1 || n_frames > pl->F) { set_error("n_frames outside [1, max_batch]"); return TOMO_EINVAL; }
     if (n_iter < 0 || n_iter >= pl->hist_cap) { set_error("n_iter outside [0, 1024]"); return TOMO_EINVAL; }
     if (pl->has_cos && !wavefront_out) { set_error("wavefront_out is NULL"); return TOMO_EINVAL; }
+    if (pl->solver_used == TOMO_SOLVER_PERSISTENT) return solve_minres_persistent(pl, slopes, wavefront_out, n_frames, n_iter, x0, (cudaStream_t)cuda_stream);
     return DISPATCH(pl, solve_minres(pl, slopes, wavefront_out, n_frames, n_iter, x0, (cudaStream_t)cuda_stream));
 }
 
@@ -837,7 +839,7 @@ extern "C" int tomo_time_phases(tomo_plan *pl, int n_frames, int n_iter, float *
     return time_phases_persistent(pl, n_frames, n_iter, us_out, (cudaStream_t)cuda_stream);
 }
 
-extern "C" int tomo_time_solver(tomo_plan *pl, const float *slopes, int n_frames, int n_iter, int reps, float *ms_out,
+extern "C" int tomo_time_solver(tomo_plan *pl, const float *slopes, int n_frames, int n_iter, int reps, int minres, float *ms_out,
                                 void *cuda_stream) {
     int rc = check_ready(pl);
     if (rc) return rc;
@@ -845,7 +847,7 @@ extern "C" int tomo_time_solver(tomo_plan *pl, const float *slopes, int n_frames
         set_error("bad arguments");
         return TOMO_EINVAL;
     }
-    return time_solver_persistent(pl, slopes, n_frames, n_iter, reps, ms_out, (cudaStream_t)cuda_stream);
+    return time_solver_persistent(pl, slopes, n_frames, n_iter, reps, minres, ms_out, (cudaStream_t)cuda_stream);
 }
 
 // ---- measurement aid: L2 read bandwidth and fp32 FMA rate of the device (tomo_measure_device)

@@ -92,7 +92,7 @@ def load(build_if_missing: bool = True):
     lib.tomo_get_zeta.argtypes = [vp, fp, C.c_int, vp]
     lib.tomo_time_kernels.argtypes = [vp, C.c_int, C.c_int, C.POINTER(C.c_float), vp]
     lib.tomo_time_phases.argtypes = [vp, C.c_int, C.c_int, C.POINTER(C.c_float), vp]
-    lib.tomo_time_solver.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_float), vp]
+    lib.tomo_time_solver.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_float), vp]
     lib.tomo_get_sizes.argtypes = [vp, ip, ip, ip, ip, ip, ip, ip]
     lib.tomo_get_valid_index.argtypes = [vp, ip, ip]
     lib.tomo_get_noise.argtypes = [vp, dp, dp]
@@ -339,9 +339,9 @@ class TomoPlan:
                          "rows", "barrier_a"),
                         [float(v) for v in us]))
 
-    def time_solver(self, slopes, n_frames: int, n_iter: int, reps: int, stream=None) -> float:
+    def time_solver(self, slopes, n_frames: int, n_iter: int, reps: int, stream=None, minres: bool = False) -> float:
         ms = (C.c_float * 1)()
-        _check(self.lib.tomo_time_solver(self._h, _ptr(slopes), n_frames, n_iter, reps, ms, _stream_handle(stream)))
+        _check(self.lib.tomo_time_solver(self._h, _ptr(slopes), n_frames, n_iter, reps, 1 if minres else 0, ms, _stream_handle(stream)))
         return float(ms[0])
 
     # -- getters --

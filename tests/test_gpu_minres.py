@@ -16,7 +16,7 @@ import pytest
 torch = pytest.importorskip("torch")
 
 from paper_1806_07938_b200 import tomo  # noqa: E402
-from test_gpu_parity import TOL_TRAJ, _horizon, dev, f32, make_plan, rel, system  # noqa: E402
+from test_gpu_parity import TOL_TRAJ, _horizon, dev, f32, make_plan, rel, solvers, system  # noqa: E402
 
 pytestmark = pytest.mark.gpu
 
@@ -30,15 +30,16 @@ def _gpu_minres(pl, s, n_it, x0=None, want_x=True):
     return d_w.cpu().numpy(), z.cpu().numpy(), pl.residuals(1, n_it)[0]
 
 
+@solvers
 @pytest.mark.parametrize("name", ["cfg1", "small_lgs", "small_odd_focus", "cfg2"])
-def test_minres_free_running_fp32_tracks_oracle_up_to_the_fp32_horizon(name):
+def test_minres_free_running_fp32_tracks_oracle_up_to_the_fp32_horizon(name, solver):
     cfg, _, osys, data = system(name)
     n_it = cfg.n_iter
     s = f32(data["slopes"][0].ravel())
     _, h64 = osys.solve_minres(s, n_it)
     _, h32 = osys.solve_minres(s, n_it, dtype=np.float32)
     k_star = max(_horizon(h32, h64) - 2, 3)
-    pl = make_plan(name)
+    pl = make_plan(name, solver=solver)
     _, _, hg = _gpu_minres(pl, s, n_it)
     d = np.abs(hg / h64 - 1.0)
     assert d[:k_star + 1].max() <= TOL_TRAJ, (name, k_star, d[:k_star + 1].max())
@@ -49,14 +50,15 @@ def test_minres_free_running_fp32_tracks_oracle_up_to_the_fp32_horizon(name):
     pl.close()
 
 
+@solvers
 @pytest.mark.parametrize("name", ["cfg1", "small_lgs", "small_fried", "ngs_offaxis", "cfg2"])
-def test_minres_converged_solution_matches_direct_solve(name):
+def test_minres_converged_solution_matches_direct_solve(name, solver):
     cfg, _, osys, data = system(name)
     s = f32(data["slopes"][0].ravel())
     zeta = osys.solve_direct(s)
     _, h = osys.solve_minres(s, 1000)
     n_it = int(np.flatnonzero(h / h[0] < 1e-6)[0])
-    pl = make_plan(name)
+    pl = make_plan(name, solver=solver)
     w, _, hg = _gpu_minres(pl, s, n_it)
     got = w.reshape(len(cfg.targets), -1)
     for t in range(len(cfg.targets)):
@@ -65,15 +67,16 @@ def test_minres_converged_solution_matches_direct_solve(name):
     pl.close()
 
 
+@solvers
 @pytest.mark.parametrize("name", ["cfg1", "small_lgs", "small_odd_focus", "cfg2"])
-def test_minres_fp64_instantiation_tracks_every_step(name):
+def test_minres_fp64_instantiation_tracks_every_step(name, solver):
     cfg, _, osys, data = system(name)
     n_it = cfg.n_iter
     s = f32(data["slopes"][0].ravel())
     _, h_a, st = osys.solve_minres(s, n_it, record=True)
     _, h_b = osys.solve_minres(s * (1.0 + 1e-15 * np.cos(np.arange(s.size))), n_it)
     k_rep = max(min(_horizon(h_b, h_a, tol=1e-4) - 2, n_it), 3)
-    pl = make_plan(name, precision=tomo.TOMO_F64)
+    pl = make_plan(name, precision=tomo.TOMO_F64, solver=solver)
     _, _, hg = _gpu_minres(pl, s, k_rep)
     assert np.abs(hg / h_a[:k_rep + 1] - 1.0).max() <= 1e-6, (name, k_rep, np.abs(hg / h_a[:k_rep + 1] - 1.0).max())
     for k in sorted({1, 2, 3, k_rep // 2, k_rep}):
@@ -84,9 +87,10 @@ def test_minres_fp64_instantiation_tracks_every_step(name):
     pl.close()
 
 
-def test_minres_warm_start_zero_iterations_batch_and_cg_comparison():
+@solvers
+def test_minres_warm_start_zero_iterations_batch_and_cg_comparison(solver):
     cfg, _, osys, data = system("small_lgs")
-    pl = make_plan("small_lgs", max_batch=2)
+    pl = make_plan("small_lgs", max_batch=2, solver=solver)
     s2 = data["slopes"].reshape(2, -1)
     s = f32(s2[0])
     w, z, h = _gpu_minres(pl, s, 0)
