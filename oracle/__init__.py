@@ -18,6 +18,8 @@ What it computes (each module cites the passage it follows, PAPER.md L<line>):
   toeplitz.py    the paper's 2RBT product Eq.18-28 step by step, generators, op counts
   directsum.py   matrix-free direct-sum MVM for ELT sizes (directsum.c, OpenMP)
   system.py      assembles a TomoConfig into the operator A, rhs and projections
+  layered.py     layered-phase (MCAO) variant of L199 / L516: Sigma_{phi_k s} of each layer on its meta-pupil grid from
+                 positions, no I'_k, no sum over layers; ray tracing of the layers (reading G31)
   loworder.py    low-order NGS tip/tilt path (paper-silent, L321/L412; reading G30): MMSE estimator of the aperture-mean
                  slopes from positions, tilt add-back
 
@@ -28,7 +30,9 @@ product, projector identities, CG -> Cholesky, MINRES = the least-squares minimi
 Krylov space (brute force) = scipy's minres, LGS ground-layer identity, the
 paper's printed closed-form counts (L150, L177, L197, L270, L280, L295), the telescoping
 closed form of the aperture-mean Hudgin slope variance (loworder.py); the FFT slope model against Eq.43 / Eq.46 as
-printed, summed over frequency grids refined to convergence, and against adaptive quadrature (test_oracle_fftmodel.py).
+printed, summed over frequency grids refined to convergence, and against adaptive quadrature (test_oracle_fftmodel.py);
+the layered variant against the joint Gaussian model written out sample by sample with the phase covariance, against the
+LTAO covariances through ray tracing on grid-aligned directions, and against the 2RBT product (test_oracle_layered.py).
 
 Parity unpinned: absolute WFE in nm (Table 3) and the curves of Fig.9-15 are not
 reproduced; nothing in this package depends on them.
