@@ -20,6 +20,10 @@
  *   - wavefront layout (Eq.35):
  *         [frame][target][valid phase point in row-major order of the (n+1) x (n+1) corner grid]      fp32
  *     radians of phase at the wavelength r0 is given at.
+ *   - layered-phase (MCAO) plans, tomo_options.layered != 0 (S2.D L199, S6 L516): "wavefront" is the estimate of every
+ *     LAYER on its own square grid, no pupil mask and no modal removal in layer space (reading G31):
+ *         [frame][layer k][n_m x n_m grid point, row-major, x fastest]                                fp32
+ *     grid point (mx, my) of layer k lies at ((mx, my) - (n_m - 1)/2) gamma_k d in the layer plane, centred on the axis.
  */
 #ifndef TOMO_B200_H
 #define TOMO_B200_H
@@ -97,6 +101,13 @@ typedef struct {
     int precision;                     /* TOMO_F32 | TOMO_F32S_F64A | TOMO_F64                                       */
     int solver;                        /* TOMO_SOLVER_MULTIKERNEL | TOMO_SOLVER_PERSISTENT                           */
     int build_cos;                     /* 0 = no target projection (tomo_solve then returns zeta-less zeros: EINVAL) */
+    int layered;                       /* != 0: estimate the phase of every layer on its meta-pupil grid instead of the    */
+                                       /* pupil-plane phase towards targets (L199: the new grid of Eq.16 extended over the  */
+                                       /* layer, I'_k removed, layers not summed).  geom->n_targets must be 0.  The grids   */
+                                       /* share one edge n_m (reported as n_prime by tomo_get_sizes): the smallest integer  */
+                                       /* with the parity of n+1 that is >= max_k (D + 2 h_k fov_radius)/(gamma_k d) + 1    */
+    double fov_radius;                 /* [arcsec] field radius the layer grids must cover (layered plans only; 0 = the     */
+                                       /* LTAO grid n')                                                                     */
 } tomo_options;
 
 /* Validate the problem statement (S2 L41-58; S2.F L297-333), build masks W_s, W_phi (Eq.33-35), modal matrices
@@ -143,7 +154,8 @@ int tomo_solve_minres(tomo_plan *plan, const float *slopes, float *wavefront_out
 int tomo_apply_css(tomo_plan *plan, const float *v, float *out, void *cuda_stream);
 
 /* wavefront_out = M_phi W_phi Sigma_{phi s} W_s^T M_s^T zeta  (Eq.31/32, Eq.35) for every target (A7-A8 only).
- * zeta: device fp32 [C][n_vs]; wavefront_out: device fp32 [n_targets][n_vphi]. */
+ * zeta: device fp32 [C][n_vs]; wavefront_out: device fp32 [n_targets][n_vphi].
+ * Layered plans: wavefront_out[k] = Sigma_{phi_k s} W_s^T M_s^T zeta for every layer k, device fp32 [K][n_m][n_m]. */
 int tomo_apply_cos(tomo_plan *plan, const float *zeta, float *wavefront_out, void *cuda_stream);
 
 /* One CG iteration (S2.G L337) on caller-held state, for the teacher-forced gate:
@@ -184,7 +196,8 @@ int tomo_time_solver(tomo_plan *plan, const float *slopes, int n_frames, int n_i
  * Needs no plan.  Returns TOMO_ECUDA without a device. */
 int tomo_measure_device(long long l2_bytes, int reps, float *out, void *cuda_stream);
 
-/* Sizes fixed at plan creation; any pointer may be NULL. */
+/* Sizes fixed at plan creation; any pointer may be NULL.  Layered plans: n_vphi = n_m * n_m, wavefront_len = K * n_m * n_m,
+ * n_prime = n_m. */
 int tomo_get_sizes(const tomo_plan *plan, int *n_vs, int *n_vphi, int *slopes_len, int *wavefront_len,
                    int *pad, int *pad_os, int *n_prime);
 

@@ -25,6 +25,12 @@ int tomo_host_css_generators(const tomo_geometry *geom, const tomo_cn2 *cn2, dou
 int tomo_host_cos_generators(const tomo_geometry *geom, const tomo_cn2 *cn2, double r0, double L0, int slope_model,
                              int target, double *gen_out);
 
+/* Generators of a layered plan (tomo_options.layered, L199; reading G31): xi'[k,(j,b)](l) on the n_m x n_m grid of every
+ * layer, centred on the axis: gen_out[K][C][n_m+n-1][n_m+n-1], l = q - m.  *n_m_out receives n_m for fov_radius [arcsec];
+ * gen_out may be NULL to query n_m alone.  geom->n_targets must be 0. */
+int tomo_host_layer_generators(const tomo_geometry *geom, const tomo_cn2 *cn2, double r0, double L0, int slope_model,
+                               double fov_radius, int *n_m_out, double *gen_out);
+
 /* Spectrum of one generator gen[n_out+n_in-1][n_out+n_in-1]: circular embedding at edge P, 2-D real DFT, times
  * 1/P^2, Hermitian half: spec_out[P/2+1 (kx)][P (ky)][2 (re, im)]  (L207, L265; readings G10, G24). */
 int tomo_host_generator_spectrum(const double *gen, int n_out, int n_in, int P, double *spec_out);

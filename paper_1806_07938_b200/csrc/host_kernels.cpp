@@ -302,7 +302,7 @@ void build_cos_generators(const HostModel &m, int target, std::vector<double> &g
     const double c = 1.0 / m.d;
     std::vector<Tap> st[2] = {stencil(m.slope_model, 0), stencil(m.slope_model, 1)};
     std::vector<double> tmp;
-    if (!m.lgs) tmp.assign((size_t)K * C * LL, 0.0);
+    if (!m.per_layer()) tmp.assign((size_t)K * C * LL, 0.0);
 #pragma omp parallel for collapse(2) schedule(dynamic)
     for (int k = 0; k < K; ++k)
         for (int j = 0; j < N; ++j) {
@@ -315,7 +315,7 @@ void build_cos_generators(const HostModel &m, int target, std::vector<double> &g
                 std::vector<std::complex<double>> tab;
                 for (int b = 0; b < 2; ++b) {
                     fft_model_table(NG, w, m.gamma[k], m.r0, m.L0, shx, shy, 3 + b, tab);
-                    double *o = m.lgs ? &gen[((size_t)k * C + 2 * j + b) * LL] : &tmp[((size_t)k * C + 2 * j + b) * LL];
+                    double *o = m.per_layer() ? &gen[((size_t)k * C + 2 * j + b) * LL] : &tmp[((size_t)k * C + 2 * j + b) * LL];
                     for (int ly = -(np - 1); ly < n; ++ly)
                         for (int lx = -(np - 1); lx < n; ++lx)
                             o[(size_t)(ly + np - 1) * Los + (lx + np - 1)] =
@@ -326,7 +326,7 @@ void build_cos_generators(const HostModel &m, int target, std::vector<double> &g
             Lattice lat(-2 * np, 2 * n, 0.5 * w, shx, shy, m.r0, m.L0);
             const double scale = m.frac[k] * (-0.5 * c);
             for (int b = 0; b < 2; ++b) {
-                double *o = m.lgs ? &gen[((size_t)k * C + 2 * j + b) * LL] : &tmp[((size_t)k * C + 2 * j + b) * LL];
+                double *o = m.per_layer() ? &gen[((size_t)k * C + 2 * j + b) * LL] : &tmp[((size_t)k * C + 2 * j + b) * LL];
                 for (int ly = -(np - 1); ly < n; ++ly)
                     for (int lx = -(np - 1); lx < n; ++lx) {
                         double s = 0.0;
@@ -335,7 +335,7 @@ void build_cos_generators(const HostModel &m, int target, std::vector<double> &g
                     }
             }
         }
-    if (!m.lgs) {
+    if (!m.per_layer()) {
 #pragma omp parallel for schedule(static)
         for (long e = 0; e < (long)((size_t)C * LL); ++e) {
             double s = 0.0;

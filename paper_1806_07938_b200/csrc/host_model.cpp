@@ -75,7 +75,7 @@ bool invert_small(std::vector<double> &a, int n) {   // Gauss-Jordan with partia
 static double cone_gamma(double h, double h_gs) { return std::isinf(h_gs) ? 1.0 : (h_gs - h) / h_gs; }
 
 int build_model(const tomo_geometry *g, const tomo_cn2 *cn2, double r0, double L0, const tomo_noise *noise,
-                int slope_model, int pad, int pad_os, HostModel &m, std::string &err) {
+                int slope_model, int pad, int pad_os, HostModel &m, std::string &err, int layered, double fov_radius_arcsec) {
     if (!g || !cn2) { err = "geometry / cn2 is NULL"; return TOMO_EINVAL; }
     if (g->n < 2 || g->n > 512 || !(g->D > 0)) { err = "need 2 <= n <= 512 and D > 0"; return TOMO_EINVAL; }
     if (g->n_wfs < 1 || g->n_wfs > 16 || !g->wfs) { err = "need 1 <= n_wfs <= 16"; return TOMO_EINVAL; }
@@ -85,6 +85,8 @@ int build_model(const tomo_geometry *g, const tomo_cn2 *cn2, double r0, double L
     if (g->n_lo < 0 || (g->n_lo > 0 && !g->lo_wfs)) { err = "bad low-order sensor list"; return TOMO_EINVAL; }
     if (slope_model != TOMO_HUDGIN && slope_model != TOMO_FRIED && slope_model != TOMO_FFTMODEL) { err = "unknown slope model"; return TOMO_EINVAL; }
     if (g->obstruction < 0 || g->obstruction >= 1) { err = "obstruction must be in [0,1)"; return TOMO_EINVAL; }
+    if (layered && g->n_targets != 0) { err = "a layered plan estimates layers, not targets: n_targets must be 0"; return TOMO_EINVAL; }
+    if (layered && !(fov_radius_arcsec >= 0)) { err = "fov_radius must be >= 0"; return TOMO_EINVAL; }
     m = HostModel();
     m.n = g->n; m.D = g->D; m.d = g->D / g->n; m.r0 = r0; m.L0 = L0; m.obstruction = g->obstruction;
     m.n_wfs = g->n_wfs; m.C = 2 * g->n_wfs; m.K = cn2->n_layers; m.T = g->n_targets; m.slope_model = slope_model;
@@ -111,7 +113,9 @@ int build_model(const tomo_geometry *g, const tomo_cn2 *cn2, double r0, double L
         fsum += fk;
     }
     if (std::fabs(fsum - 1.0) > 1e-9) { err = "Cn2 fractions do not sum to 1"; return TOMO_EINVAL; }
-    for (int t = 0; t < m.T; ++t) { m.bx.push_back(g->target_xy[2 * t] * kArcsec); m.by.push_back(g->target_xy[2 * t + 1] * kArcsec); }
+    m.layered = layered != 0;
+    if (m.layered) { m.T = 1; m.bx.push_back(0.0); m.by.push_back(0.0); }   // the grid of Eq.16 with beta = 0 (reading G31)
+    else for (int t = 0; t < m.T; ++t) { m.bx.push_back(g->target_xy[2 * t] * kArcsec); m.by.push_back(g->target_xy[2 * t + 1] * kArcsec); }
 
     // masks: subaperture valid iff its centre is inside the pupil (reading G12); phase point valid iff it is a
     // corner of a valid subaperture (Fig.2)
@@ -148,12 +152,17 @@ int build_model(const tomo_geometry *g, const tomo_cn2 *cn2, double r0, double L
     m.nvp = (int)m.ph_idx.size();
 
     // n' (L179, L295; reading G19): smallest integer >= n/gamma_min + 1 with the parity of n+1
+    // layered plans (L199; reading G31): the grid covers the meta-pupil D + 2 h_k theta of every layer at spacing gamma_k d
     {
-        int np = (int)std::ceil(n / gmin + 1.0 - 1e-9);
+        double v = n / gmin + 1.0;
+        if (m.layered)
+            for (int k = 0; k < m.K; ++k)
+                v = std::max(v, (m.D + 2.0 * m.h[k] * fov_radius_arcsec * kArcsec) / (m.gamma[k] * m.d) + 1.0);
+        int np = (int)std::ceil(v - 1e-9);
         if ((np - (n + 1)) % 2 != 0) ++np;
         m.n_p = np;
     }
-    m.Kp = m.lgs ? m.K : 1;
+    m.Kp = m.per_layer() ? m.K : 1;
     m.P = pad > 0 ? pad : next_fft_size(2 * n - 1);
     m.P_os = pad_os > 0 ? pad_os : next_fft_size(m.n_p + n - 1);
     if (m.P % 2 || !is_5smooth(m.P) || m.P_os % 2 || !is_5smooth(m.P_os)) {
@@ -223,6 +232,7 @@ int build_model(const tomo_geometry *g, const tomo_cn2 *cn2, double r0, double L
             for (int e = 0; e < 2 * m.nv; ++e) m.sigma2_full[(size_t)2 * i * m.nv + e] = s2;
         }
     }
+    m.out_len = m.layered ? (size_t)m.Kp * m.n_p * m.n_p : (size_t)m.T * m.nvp;
     // I'_k (Eq.16; readings G18-G19): per-axis bilinear taps of the original phase points on the n' grid of
     // spacing d_k centred on the target footprint: position r_p/d_k + (n'-1)/2, independent of the target
     m.interp_i0.assign((size_t)m.Kp * (n + 1), 0);

@@ -18,6 +18,9 @@ struct HostModel {
     int n = 0, n_wfs = 0, C = 0, K = 0, T = 0;
     double D = 0, d = 0, r0 = 0, L0 = 0, h_gs = 0, obstruction = 0;
     bool lgs = false;
+    bool layered = false;                // layered-phase (MCAO) plan (L199; reading G31): T = 1 pseudo-target on the axis,
+                                         // layers kept apart, n_p = n_m, no I'_k / W_phi / M_phi
+    bool per_layer() const { return lgs || layered; }
     int slope_model = TOMO_HUDGIN;
     std::vector<double> ax, ay;          // WFS directions [rad]
     std::vector<double> bx, by;          // target directions [rad]
@@ -32,7 +35,8 @@ struct HostModel {
     int nv = 0, nvp = 0;
     // FFT sizes
     int n_p = 0;                         // n' (L179, L295; reading G19)
-    int Kp = 0;                          // layers kept apart in the phi-s product: K (LGS) or 1 (NGS)
+    int Kp = 0;                          // layers kept apart in the phi-s product: K (LGS, layered) or 1 (NGS)
+    size_t out_len = 0;                  // fp32 values one frame's projection writes: T * nvp, layered: K * n_p * n_p
     int P = 0, Ph = 0, P_os = 0, Ph_os = 0, n_pair = 0;
     // mode removal (Eq.36): per WFS G = (Z^T Z)^-1, row-major 3x3 (unused rows/cols zero)
     std::vector<double> Gs;              // [n_wfs][9]
@@ -50,7 +54,8 @@ struct HostModel {
 
 // Fill a HostModel from the ABI structs; returns TOMO_OK or an error code and sets `err`.
 int build_model(const tomo_geometry *g, const tomo_cn2 *cn2, double r0, double L0, const tomo_noise *noise,
-                int slope_model, int pad, int pad_os, HostModel &m, std::string &err);
+                int slope_model, int pad, int pad_os, HostModel &m, std::string &err, int layered = 0,
+                double fov_radius_arcsec = 0.0);
 
 // D_phi(r) of Eq.53 (L619) with the exact prefactor (reading G2).
 double structure_function(double r, double r0, double L0);

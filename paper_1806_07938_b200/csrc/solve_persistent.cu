@@ -242,7 +242,7 @@ int solve_persistent(tomo_plan *pl, const float *slopes, float *out, int F, int 
     if ((rc = persist_dispatch(pl, st, F, n_iter, x0 ? PM_WARM : PM_COLD, 0, slopes, x0, nullptr))) return rc;
     if (pl->has_cos && out) {
         if ((rc = project_from_x(pl, st, F))) return rc;
-        PCK(cudaMemcpyAsync(out, pl->d_out, (size_t)F * pl->m.T * pl->m.nvp * sizeof(float), cudaMemcpyDeviceToDevice, st));
+        PCK(cudaMemcpyAsync(out, pl->d_out, (size_t)F * pl->m.out_len * sizeof(float), cudaMemcpyDeviceToDevice, st));
     }
     pl->last_frames = F; pl->last_iter = n_iter;
     return TOMO_OK;
@@ -257,7 +257,7 @@ int solve_minres_persistent(tomo_plan *pl, const float *slopes, float *out, int 
     if ((rc = persist_dispatch(pl, st, F, n_iter, x0 ? PM_WARM : PM_COLD, 0, slopes, x0, nullptr, nullptr, METHOD_MINRES))) return rc;
     if (pl->has_cos && out) {
         if ((rc = project_from_x(pl, st, F))) return rc;
-        PCK(cudaMemcpyAsync(out, pl->d_out, (size_t)F * pl->m.T * pl->m.nvp * sizeof(float), cudaMemcpyDeviceToDevice, st));
+        PCK(cudaMemcpyAsync(out, pl->d_out, (size_t)F * pl->m.out_len * sizeof(float), cudaMemcpyDeviceToDevice, st));
     }
     pl->last_frames = F; pl->last_iter = n_iter;
     return TOMO_OK;

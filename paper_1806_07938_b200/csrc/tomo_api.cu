@@ -105,7 +105,7 @@ extern "C" int tomo_plan_create(const tomo_geometry *geom, const tomo_cn2 *cn2, 
     tomo_plan *pl = new (std::nothrow) tomo_plan();
     if (!pl) { set_error("out of host memory"); return TOMO_ENOMEM; }
     std::string err;
-    int rc = build_model(geom, cn2, r0, L0, noise, opt.slope_model, opt.pad, opt.pad_os, pl->m, err);
+    int rc = build_model(geom, cn2, r0, L0, noise, opt.slope_model, opt.pad, opt.pad_os, pl->m, err, opt.layered, opt.fov_radius);
     if (rc) { set_error(err); delete pl; return rc; }
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
@@ -173,7 +173,7 @@ extern "C" int tomo_plan_create(const tomo_geometry *geom, const tomo_cn2 *cn2, 
         TRY(dev_alloc_bytes(pl, &pl->d_T2os, Fc * m.T * m.Kp * m.Ph_os * m.n_p * 2 * E));
         TRY(dev_alloc_bytes(pl, &pl->d_G, Fc * m.T * m.Kp * m.n_p * m.n_p * E));
         TRY(dev_alloc_bytes(pl, &pl->d_phi, F * m.T * m.nvp * E));
-        TRY(dev_alloc<float>(pl, &pl->d_out, F * m.T * m.nvp));
+        TRY(dev_alloc<float>(pl, &pl->d_out, F * m.out_len));
         TRY(dev_alloc_bytes(pl, &pl->d_spec_os, (size_t)m.T * m.Kp * m.Ph_os * m.C * m.P_os * 2 * pl->selem));
     }
 #undef TRY
@@ -373,6 +373,14 @@ template <typename T, typename S> struct Ops {
             r.st = so; r.g = pl->g; r.F = Fn; r.T2 = (const C2 *)pl->d_T2os; r.G = (T *)pl->d_G;
             k_cos_rows_inv<T><<<grid_for(Fn * m.T * m.Kp * ((m.n_p + 1) / 2), kRowWarps), 32 * kRowWarps, rs, st>>>(r);
             LAUNCH_CHECK();
+            if (m.layered) {        // L199: the layer grids ARE the result -- no I'_k, no sum over layers, no W_phi / M_phi
+                const size_t cnt = (size_t)Fn * m.out_len;
+                k_convert<T, float><<<(unsigned)std::min<size_t>((cnt + 255) / 256, 148 * 8), 256, 0, st>>>(
+                    (const T *)pl->d_G, pl->d_out + (size_t)f0 * m.out_len, cnt);
+                LAUNCH_CHECK();
+                pl->launches_last += 5;
+                continue;
+            }
             const size_t total = (size_t)Fn * m.T * m.nvp;
             k_cos_gather<T><<<(unsigned)std::min<size_t>((total * 8 + 255) / 256, 148 * 8), 256, 0, st>>>(
                 pl->g, Fn, (const T *)pl->d_G, pl->d_interp_i0, (const T *)pl->d_interp_w,
@@ -380,6 +388,7 @@ template <typename T, typename S> struct Ops {
             LAUNCH_CHECK();
             pl->launches_last += 5;
         }
+        if (m.layered) return TOMO_OK;
         k_phase_project<T><<<dim3(m.T, F), 1024, 0, st>>>(pl->g, (const T *)pl->d_phi, pl->d_out);
         LAUNCH_CHECK();
         pl->launches_last += 1;
@@ -467,7 +476,7 @@ template <typename T, typename S> struct Ops {
             CK(cudaGraphLaunch(it->second, st));
         }
         if (with_cos)
-            CK(cudaMemcpyAsync(out, pl->d_out, (size_t)F * m.T * m.nvp * sizeof(float), cudaMemcpyDeviceToDevice, st));
+            CK(cudaMemcpyAsync(out, pl->d_out, (size_t)F * m.out_len * sizeof(float), cudaMemcpyDeviceToDevice, st));
         pl->last_frames = F; pl->last_iter = n_iter;
         return TOMO_OK;
     }
@@ -564,7 +573,7 @@ template <typename T, typename S> struct Ops {
         }
         CK(cudaGraphLaunch(it->second, st));
         if (with_cos)
-            CK(cudaMemcpyAsync(out, pl->d_out, (size_t)F * m.T * m.nvp * sizeof(float), cudaMemcpyDeviceToDevice, st));
+            CK(cudaMemcpyAsync(out, pl->d_out, (size_t)F * m.out_len * sizeof(float), cudaMemcpyDeviceToDevice, st));
         pl->last_frames = F; pl->last_iter = n_iter;
         return TOMO_OK;
     }
@@ -596,7 +605,7 @@ template <typename T, typename S> struct Ops {
         LAUNCH_CHECK();
         pl->launches_last += 1;
         if ((rc = project_targets(pl, st, 1))) return rc;
-        CK(cudaMemcpyAsync(out, pl->d_out, (size_t)pl->m.T * pl->m.nvp * sizeof(float), cudaMemcpyDeviceToDevice, st));
+        CK(cudaMemcpyAsync(out, pl->d_out, pl->m.out_len * sizeof(float), cudaMemcpyDeviceToDevice, st));
         return TOMO_OK;
     }
 
@@ -934,9 +943,9 @@ extern "C" int tomo_get_sizes(const tomo_plan *pl, int *n_vs, int *n_vphi, int *
                               int *pad, int *pad_os, int *n_prime) {
     if (!pl) { set_error("plan is NULL"); return TOMO_EINVAL; }
     if (n_vs) *n_vs = pl->m.nv;
-    if (n_vphi) *n_vphi = pl->m.nvp;
+    if (n_vphi) *n_vphi = pl->m.layered ? pl->m.n_p * pl->m.n_p : pl->m.nvp;
     if (slopes_len) *slopes_len = pl->m.C * pl->m.nv;
-    if (wavefront_len) *wavefront_len = pl->m.T * pl->m.nvp;
+    if (wavefront_len) *wavefront_len = (int)pl->m.out_len;
     if (pad) *pad = pl->m.P;
     if (pad_os) *pad_os = pl->m.P_os;
     if (n_prime) *n_prime = pl->m.n_p;
@@ -1026,6 +1035,21 @@ extern "C" int tomo_host_cos_generators(const tomo_geometry *g, const tomo_cn2 *
     if (target < 0 || target >= m.T) { set_error("target out of range"); return TOMO_EINVAL; }
     std::vector<double> gen;
     build_cos_generators(m, target, gen);
+    std::memcpy(gen_out, gen.data(), gen.size() * sizeof(double));
+    return TOMO_OK;
+}
+
+extern "C" int tomo_host_layer_generators(const tomo_geometry *g, const tomo_cn2 *cn2, double r0, double L0, int slope_model,
+                                          double fov_radius, int *n_m_out, double *gen_out) {
+    HostModel m;
+    std::string err;
+    tomo_noise nz; std::memset(&nz, 0, sizeof(nz));
+    int rc = build_model(g, cn2, r0, L0, &nz, slope_model, 0, 0, m, err, 1, fov_radius);
+    if (rc) { set_error(err); return rc; }
+    if (n_m_out) *n_m_out = m.n_p;
+    if (!gen_out) return TOMO_OK;
+    std::vector<double> gen;
+    build_cos_generators(m, 0, gen);
     std::memcpy(gen_out, gen.data(), gen.size() * sizeof(double));
     return TOMO_OK;
 }

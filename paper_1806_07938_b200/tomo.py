@@ -26,7 +26,8 @@ EXPORTS = (
     "tomo_apply_cos", "tomo_cg_step", "tomo_get_zeta", "tomo_time_kernels", "tomo_time_phases", "tomo_time_solver", "tomo_measure_device",
     "tomo_get_sizes", "tomo_get_valid_index", "tomo_get_noise",
     "tomo_get_residuals", "tomo_get_stats", "tomo_get_solver", "tomo_plan_destroy", "tomo_last_error",
-    "tomo_host_sizes", "tomo_host_css_generators", "tomo_host_cos_generators", "tomo_host_generator_spectrum",
+    "tomo_host_sizes", "tomo_host_css_generators", "tomo_host_cos_generators", "tomo_host_layer_generators",
+    "tomo_host_generator_spectrum",
     "tomo_host_structure_function", "tomo_host_slab_segments",
     "tomo_host_lo_estimator", "tomo_lo_create", "tomo_lo_apply", "tomo_lo_destroy",
 )
@@ -60,7 +61,8 @@ class _Noise(C.Structure):
 
 class _Options(C.Structure):
     _fields_ = [("slope_model", C.c_int), ("pad", C.c_int), ("pad_os", C.c_int), ("max_batch", C.c_int),
-                ("precision", C.c_int), ("solver", C.c_int), ("build_cos", C.c_int)]
+                ("precision", C.c_int), ("solver", C.c_int), ("build_cos", C.c_int), ("layered", C.c_int),
+                ("fov_radius", C.c_double)]
 
 
 _lib = None
@@ -105,6 +107,8 @@ def load(build_if_missing: bool = True):
     lib.tomo_host_css_generators.argtypes = [C.POINTER(_Geometry), C.POINTER(_Cn2), C.c_double, C.c_double, C.c_int, dp]
     lib.tomo_host_cos_generators.argtypes = [C.POINTER(_Geometry), C.POINTER(_Cn2), C.c_double, C.c_double, C.c_int,
                                              C.c_int, dp]
+    lib.tomo_host_layer_generators.argtypes = [C.POINTER(_Geometry), C.POINTER(_Cn2), C.c_double, C.c_double, C.c_int,
+                                               C.c_double, ip, dp]
     lib.tomo_host_generator_spectrum.argtypes = [dp, C.c_int, C.c_int, C.c_int, dp]
     lib.tomo_host_structure_function.argtypes = [dp, C.c_int, C.c_double, C.c_double, dp]
     lib.tomo_measure_device.argtypes = [C.c_longlong, C.c_int, C.POINTER(C.c_float), vp]
@@ -132,12 +136,12 @@ def _dp(a: np.ndarray):
 class _Problem:
     """Keeps the numpy arrays behind the ABI structs alive."""
 
-    def __init__(self, cfg, subap_mask: Optional[np.ndarray] = None):
+    def __init__(self, cfg, subap_mask: Optional[np.ndarray] = None, no_targets: bool = False):
         self.cfg = cfg
         self.wfs = (_Wfs * len(cfg.wfs))(*[_Wfs(w.ax, w.ay, w.h_gs, w.n_remove) for w in cfg.wfs])
         lo = getattr(cfg, "lo_wfs", ())
         self.lo = (_Wfs * max(len(lo), 1))(*[_Wfs(w.ax, w.ay, w.h_gs, w.n_remove) for w in lo])
-        self.targets = np.ascontiguousarray(np.asarray(cfg.targets, dtype=np.float64).reshape(-1, 2))
+        self.targets = np.ascontiguousarray(np.asarray(() if no_targets else cfg.targets, dtype=np.float64).reshape(-1, 2))
         self.h = np.ascontiguousarray(cfg.h, dtype=np.float64)
         self.frac = np.ascontiguousarray(cfg.frac, dtype=np.float64)
         self.mask = None if subap_mask is None else np.ascontiguousarray(subap_mask, dtype=np.uint8)
@@ -174,6 +178,18 @@ def host_cos_generators(cfg, target: int = 0, slope_model: int = TOMO_HUDGIN) ->
     out = np.empty((sz["Kp"], Cc, L, L), dtype=np.float64)
     _check(lib.tomo_host_cos_generators(pr.geom, pr.cn2, cfg.r0, cfg.L0, slope_model, target, _dp(out)))
     return out
+
+
+def host_layer_generators(cfg, fov_radius: float, slope_model: int = TOMO_HUDGIN):
+    """(n_m, xi'[K][C][n_m+n-1][n_m+n-1]) of a layered plan (L199; reading G31)."""
+    lib = load()
+    pr = _Problem(cfg, no_targets=True)
+    nm = C.c_int()
+    _check(lib.tomo_host_layer_generators(pr.geom, pr.cn2, cfg.r0, cfg.L0, slope_model, fov_radius, C.byref(nm), None))
+    L = nm.value + cfg.n - 1
+    out = np.empty((len(cfg.h), 2 * len(cfg.wfs), L, L), dtype=np.float64)
+    _check(lib.tomo_host_layer_generators(pr.geom, pr.cn2, cfg.r0, cfg.L0, slope_model, fov_radius, C.byref(nm), _dp(out)))
+    return nm.value, out
 
 
 def host_generator_spectrum(gen: np.ndarray, n_out: int, n_in: int, P: int) -> np.ndarray:
@@ -269,10 +285,14 @@ class TomoPlan:
     def __init__(self, cfg, *, noise_frac: Optional[float] = None, sigma2_wfs: Optional[Sequence[float]] = None,
                  sigma2_subap=None, sigma_xy_subap=None, slope_model: int = TOMO_HUDGIN, max_batch: int = 1, precision: int = TOMO_F32,
                  solver: int = TOMO_SOLVER_PERSISTENT, build_cos: bool = True, subap_mask=None,
-                 css_gen: Optional[np.ndarray] = None, cos_gen: Optional[np.ndarray] = None, upload: bool = True):
+                 css_gen: Optional[np.ndarray] = None, cos_gen: Optional[np.ndarray] = None, upload: bool = True,
+                 layered: bool = False, fov_radius: float = 0.0):
+        """layered=True: the plan estimates every layer on its meta-pupil grid (tomo_options.layered, L199); the targets of
+        cfg are ignored and the "wavefront" of the solves is [frame][layer][n_prime][n_prime]."""
         self.lib = load()
         self.cfg = cfg
-        self._pr = _Problem(cfg, subap_mask)
+        self.layered = bool(layered)
+        self._pr = _Problem(cfg, subap_mask, no_targets=self.layered)
         if sigma2_subap is not None:
             self._s2 = np.ascontiguousarray(sigma2_subap, dtype=np.float64)
             self._sxy = None if sigma_xy_subap is None else np.ascontiguousarray(sigma_xy_subap, dtype=np.float64)
@@ -282,13 +302,14 @@ class TomoPlan:
             noise = _Noise(_dp(self._s2), 0.0, None, None)
         else:
             noise = _Noise(None, cfg.noise_frac if noise_frac is None else noise_frac, None, None)
-        opt = _Options(slope_model, cfg.pad, cfg.pad_os, max_batch, precision, solver, 1 if build_cos else 0)
+        opt = _Options(slope_model, cfg.pad, 0 if self.layered else cfg.pad_os, max_batch, precision, solver,
+                       1 if build_cos else 0, 1 if self.layered else 0, float(fov_radius))
         self._h = C.c_void_p()
         _check(self.lib.tomo_plan_create(self._pr.geom, self._pr.cn2, cfg.r0, cfg.L0, noise, opt, C.byref(self._h)))
         v = [C.c_int() for _ in range(7)]
         _check(self.lib.tomo_get_sizes(self._h, *[C.byref(x) for x in v]))
         (self.n_vs, self.n_vphi, self.slopes_len, self.wavefront_len, self.P, self.P_os, self.n_prime) = [x.value for x in v]
-        self.n_targets = len(cfg.targets)
+        self.n_targets = len(cfg.h) if self.layered else len(cfg.targets)     # layered: one n_prime^2 grid per layer
         self.n_wfs = len(cfg.wfs)
         self.max_batch = max_batch
         self.has_cos = build_cos and self.n_targets > 0

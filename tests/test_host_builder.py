@@ -2,6 +2,7 @@
 oracle's independent evaluation of the same paper formulas (Eq.50-53)."""
 import math
 import os
+from dataclasses import replace
 
 import numpy as np
 import pytest
@@ -83,6 +84,25 @@ def test_generators_match_oracle(name, model):
     g2 = tomo.host_cos_generators(cfg, 0, model)
     assert g2.shape == xi.shape
     assert np.abs(g2 - xi).max() <= 1e-11 * np.abs(xi).max()
+
+
+@pytest.mark.parametrize("model", [tomo.TOMO_HUDGIN, tomo.TOMO_FRIED])
+@pytest.mark.parametrize("name", ["cfg1", "small_lgs"])
+def test_layered_plan_generators_and_grid_edge_match_oracle(name, model):
+    """Layered (MCAO) plans, L199 / reading G31: n_m from the field radius and the per-layer generators on the axis-centred
+    n_m grid (NGS systems keep their layers apart too) against oracle/layered.py + toeplitz.cos_generators at beta = 0."""
+    from oracle import layered as lay
+    cfg = (replace(get_config("cfg1"), h=(0.0, 4000.0, 11000.0), frac=(0.55, 0.25, 0.2)) if name == "cfg1"
+           else small_lgs_config(n=9, n_gs=3, n_layers=3))
+    mname = {tomo.TOMO_HUDGIN: "hudgin", tomo.TOMO_FRIED: "fried"}[model]
+    dirs, hgs = [(w.ax, w.ay) for w in cfg.wfs], cfg.wfs[0].h_gs
+    for fov in (0.0, 25.0, 60.0):
+        n_m, g = tomo.host_layer_generators(cfg, fov, model)
+        assert n_m == lay.n_meta(cfg.n, cfg.d, cfg.h, hgs, fov)
+        xi = tz.cos_generators(cfg.n, n_m, cfg.d, dirs, hgs, (0.0, 0.0), cfg.h, cfg.frac, cfg.r0, cfg.L0, mname)
+        xi = xi.reshape(len(cfg.h), 2 * len(dirs), xi.shape[-1], xi.shape[-1])
+        assert g.shape == xi.shape and np.abs(g - xi).max() <= 1e-11 * np.abs(xi).max()
+    assert tomo.host_layer_generators(cfg, 0.0, model)[0] == tomo.host_sizes(cfg)["n_prime"]
 
 
 @pytest.mark.parametrize("name", ["cfg1", "small_lgs"])
