@@ -172,14 +172,15 @@ int tomo_get_zeta(tomo_plan *plan, float *zeta_out, int n_frames, void *cuda_str
  * update.  The state of the last solve is overwritten. */
 int tomo_time_kernels(tomo_plan *plan, int n_frames, int n_iter, float *ms_out, void *cuda_stream);
 
-/* Measurement aid for the persistent solver: one instrumented solve of n_iter iterations from the state the last
- * solve left in the plan; thread 0 of every CTA stamps the SM cycle counter at the phase boundaries.  Synchronises
+/* Measurement aid for the persistent solver: one instrumented solve of n_iter iterations -- CG (minres = 0) from the state
+ * the last solve left in the plan, MINRES (minres != 0; TOMO_F32, n_frames = 1) from a cold start on the projected slopes
+ * of the last solve; thread 0 of every CTA stamps the SM cycle counter at the phase boundaries.  Synchronises
  * the stream.  us_out (host fp32 [10]), microseconds at the device's nominal SM clock, mean over iterations; work
  * segments are the maximum over CTAs, barrier segments the minimum over CTAs (= pure latency):
  * [0] whole iteration (CTA 0), [1] rho/beta scalars, [2] p~ update, [3] forward y-FFT, [4] block product,
  * [5] inverse y-FFT + T2 write, [6] grid barrier B, [7] alpha/mode scalars (+ first inverse x-FFT), [8] row phase,
  * [9] grid barrier A.  The state of the last solve is overwritten. */
-int tomo_time_phases(tomo_plan *plan, int n_frames, int n_iter, float *us_out, void *cuda_stream);
+int tomo_time_phases(tomo_plan *plan, int n_frames, int n_iter, int minres, float *us_out, void *cuda_stream);
 
 /* Measurement aid (bench.py "roofline" with the persistent solver): `reps` launches of the persistent kernel alone
  * (A1-A6: rhs projection + n_iter CG (minres = 0) or MINRES (minres != 0) iterations from a cold start on `slopes`, device fp32 [n_frames][C][n_vs]; no

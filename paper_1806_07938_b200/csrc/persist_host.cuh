@@ -80,14 +80,15 @@ static int persist_launch(tomo_plan *pl, cudaStream_t st, const PLaunch &L) {
     a.part_r = ps->d_part_r; a.part_s = ps->d_part_s; a.part_i = ps->d_part_i;
     a.hist = pl->d_hist; a.hist_stride = pl->hist_cap; a.alpha = pl->d_alpha; a.scal_out = L.scal_out;
     a.flags = ps->d_flags; a.dbg = L.dbg;
-    // the instrumented instances (tomo_time_phases) exist for TOMO_F32 and CG only; the production instances carry no stamp code
+    // the instrumented instances (tomo_time_phases) exist for TOMO_F32 only (MINRES: single frame); the production instances
+    // carry no stamp code
     const bool mr = L.method == METHOD_MINRES;
     const void *kern = mr ? (L.F > 1 ? (const void *)(k_persistent<T, S, P, true, false, METHOD_MINRES>) : (const void *)(k_persistent<T, S, P, false, false, METHOD_MINRES>))
                           : (L.F > 1 ? (const void *)(k_persistent<T, S, P, true, false, METHOD_CG>) : (const void *)(k_persistent<T, S, P, false, false, METHOD_CG>));
     if (L.dbg) {
         if constexpr (std::is_same<T, float>::value && std::is_same<S, float>::value) {
-            if (mr) { set_error("tomo_time_phases: the instrumented kernel instances run CG"); return TOMO_EUNSUPPORTED; }
-            kern = L.F > 1 ? (const void *)(k_persistent<T, S, P, true, true, METHOD_CG>) : (const void *)(k_persistent<T, S, P, false, true, METHOD_CG>);
+            if (mr && L.F > 1) { set_error("tomo_time_phases: the instrumented MINRES instance runs one frame"); return TOMO_EUNSUPPORTED; }
+            kern = mr ? (const void *)(k_persistent<T, S, P, false, true, METHOD_MINRES>) : L.F > 1 ? (const void *)(k_persistent<T, S, P, true, true, METHOD_CG>) : (const void *)(k_persistent<T, S, P, false, true, METHOD_CG>);
         } else { set_error("tomo_time_phases: the instrumented kernel instances exist for TOMO_F32 only"); return TOMO_EUNSUPPORTED; }
     }
     if (mr) { a.NQ = ps->NQ_mr; a.vec_smem = ps->vec_smem_mr; a.w1d = (T *)ps->d_w1d; a.w2d = (T *)ps->d_w2d; }

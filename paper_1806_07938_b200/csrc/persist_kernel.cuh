@@ -117,6 +117,26 @@ __device__ __forceinline__ double group_sum(double v) {
     return v;
 }
 
+// Modal sums against G = (Z^T Z)^-1 of one WFS (3 x 3, rows / columns beyond n_remove are zero; Eq.36).  The loops run
+// to the constant 3 under a predicate so that the three-element arrays stay in registers: a loop to n_remove indexes them
+// dynamically and sends them to local memory (measured: 3 us per MINRES iteration at cfg3).
+__device__ __forceinline__ double modal_quad(const double *G, const double tp[3], const double tq[3], int nr) {
+    double t = 0.0;
+#pragma unroll
+    for (int u = 0; u < 3; ++u) {
+        double sq = 0.0;
+#pragma unroll
+        for (int v = 0; v < 3; ++v) if (v < nr) sq += G[u * 3 + v] * tq[v];
+        if (u < nr) t += tp[u] * sq;
+    }
+    return t;
+}
+__device__ __forceinline__ void modal_coef(const double *G, const double tq[3], int nr, int comp, double &d0, double &d2) {
+    d0 = 0.0; d2 = 0.0;
+#pragma unroll
+    for (int v = 0; v < 3; ++v) if (v < nr) { d0 += G[comp * 3 + v] * tq[v]; d2 += G[6 + v] * tq[v]; }
+}
+
 // deterministic sum by one warp of up to 160 contiguous doubles other CTAs wrote: all loads in flight at once
 __device__ __forceinline__ double warp_sum_cg160(const double *src, int count, int lane) {
     double v[5];
@@ -560,20 +580,16 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
         if (b == 0) a.hist[(size_t)f * a.hist_stride + kk] = st[MR_PHIBAR] * st[MR_PHIBAR];
     };
 
-    // MINRES: alpha_k = v_k . M_s q = v.q - (Z^T v)^T (Z^T Z)^-1 Z^T q from the Parseval sums of one frame
+    // MINRES: alpha_k = v_k . M_s q = v.q - (Z^T v)^T (Z^T Z)^-1 Z^T q from the Parseval sums of one frame: one WFS term per
+    // lane of a 16-lane group, summed in the group's fixed order (called by whole groups)
     auto minres_alpha = [&](const double *sc) {
-        double al = sc[SC_PQ];
         const double *S0 = sc + SC_HEAD, *S1 = S0 + C, *V0 = sc + SCM, *V1 = V0 + C;
-        for (int i = 0; i < N; ++i) {
-            const int nr = s_nrem[i];
+        double term = 0.0;
+        for (int i = gl; i < N; i += kGS) {
             const double tq[3] = {S0[2 * i], S0[2 * i + 1], S1[2 * i] + S1[2 * i + 1]}, tp[3] = {V0[2 * i], V0[2 * i + 1], V1[2 * i] + V1[2 * i + 1]};
-            for (int u = 0; u < nr; ++u) {
-                double sq = 0.0;
-                for (int v = 0; v < nr; ++v) sq += sGs[i * 9 + u * 3 + v] * tq[v];
-                al -= tp[u] * sq;
-            }
+            term += modal_quad(sGs + i * 9, tp, tq, s_nrem[i]);
         }
-        return al;
+        return sc[SC_PQ] - group_sum(term);
     };
 
     // ================================================================ iterations (k = -1 is the warm-start product A x0)
@@ -694,14 +710,16 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
             PSTAMP(PT_MAC);
             // inverse y-FFT as a forward transform of conj(y~): pass 1 Ubuf -> Vbuf; the warps without pass-1 items
             // reduce the slab partials meanwhile
-            if (p1) dft_pass<T, A, true>(Ubuf + c1 * LD + j2s, B, A, Vbuf + c1 * LD + j2s, B + 1, tw, j2s);
-            {
-                const int WPG = (P + 31) >> 5, Goc = min(NW / WPG, C);
-                // (batch: every warp takes its share once its pass-1 column is done; with two frames only 4 warps are free)
-                const int wb = (nf * C * B + 31) >> 5, nfree = (!BATCH && (NW - wb) > 0) ? NW - wb : NW;
-                const int slot = NW - 1 - warp;             // free warps are the top ones
+            // The warps without pass items reduce the slab partials meanwhile (from the top warp down): the first n_pub1 items beside
+            // pass 1, the rest beside pass 2 (which keeps fewer warps busy), so that neither window holds more than ~one trip
+            const int WPG = (P + 31) >> 5, Goc = min(NW / WPG, C);
+            const int wb1 = (nf * C * B + 31) >> 5, wb2 = (nf * C * A + 31) >> 5;
+            const int free1 = (!BATCH && NW - wb1 > 0) ? NW - wb1 : NW, free2 = (!BATCH && NW - wb2 > 0) ? NW - wb2 : NW;
+            const int n_pub = nf * NQ, n_pub1 = (BATCH || n_pub <= free1) ? n_pub : max(free1, n_pub - free2);
+            auto publish = [&](int lo, int hi, int nfree) {
+                const int slot = NW - 1 - warp;
                 if (slot < nfree) {
-                    for (int tq = slot; tq < nf * NQ; tq += nfree) {
+                    for (int tq = lo + slot; tq < hi; tq += nfree) {
                         const int fr = tq / NQ, q1 = tq - fr * NQ;
                         const T *rd = red + fr * red_sz;
                         double s = 0.0;
@@ -710,9 +728,12 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                         if (lane == 0) a.part_s[((size_t)(f0 + fr) * NQ + q1) * Ph + kxi] = (double)wkx * s;
                     }
                 }
-            }
+            };
+            if (p1) dft_pass<T, A, true>(Ubuf + c1 * LD + j2s, B, A, Vbuf + c1 * LD + j2s, B + 1, tw, j2s);
+            publish(0, n_pub1, free1);
             __syncthreads();
             if (p2) dft_pass<T, B, false>(Vbuf + c2s * LD + k1s * (B + 1), 1, B, Ubuf + c2s * LD + k1s, A, tw, 0);
+            publish(n_pub1, n_pub, free2);
             __syncthreads();
             // batch: the T1 / T1p loads of the next pass fly during this pass's T2 store
             if (BATCH && it + nf < n_items) prefetch_slab(it + nf, !take_new);
@@ -807,12 +828,21 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                 // alpha_k is recorded for the next phase C / the tail; every row unit derives alpha and its own mode
                 // coefficients from the sums itself (a few fp64 operations per lane beat a serial section + a barrier)
                 if (!pre) {
-                    for (int f = tid; f < F; f += kPThreads) {
-                        double *sc = scal + f * SB;
-                        const double rho = sc[SC_RHO], pq = sc[SC_PQ];
-                        const double al = MINRES ? minres_alpha(sc) : (rho > 0.0 && pq > 0.0) ? div_as<T>(rho, pq) : 0.0;     // breakdown: freeze (reading G16)
-                        sc[SC_ALPHA] = al;
-                        if (b == 0) a.alpha[f] = al;
+                    if (MINRES && BATCH) {                                       // (single frame: recorded in stage 2 below)
+                        for (int f0 = gs & ~1; f0 < F; f0 += kPThreads / kGS) {   // one 16-lane group per frame; the two groups of a
+                            const int f = f0 + (gs & 1);                         // warp go through the full-mask shuffles together
+                            double *sc = scal + min(f, F - 1) * SB;
+                            const double al = minres_alpha(sc);
+                            if (gl == 0 && f < F) { sc[SC_ALPHA] = al; if (b == 0) a.alpha[f] = al; }
+                        }
+                    } else if (!MINRES) {
+                        for (int f = tid; f < F; f += kPThreads) {
+                            double *sc = scal + f * SB;
+                            const double rho = sc[SC_RHO], pq = sc[SC_PQ];
+                            const double al = (rho > 0.0 && pq > 0.0) ? div_as<T>(rho, pq) : 0.0;     // breakdown: freeze (reading G16)
+                            sc[SC_ALPHA] = al;
+                            if (b == 0) a.alpha[f] = al;
+                        }
                     }
                 }
                 PSTAMP(PT_SCAL);
@@ -821,18 +851,8 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
             double rr = 0.0;
             double al_mr = 0.0;                      // MINRES: alpha_k of the unit's frame, one WFS term per lane of the group
             if (MINRES && !pre) {
-                const double *sc = scal + q.f * SB, *S0 = sc + SC_HEAD, *S1 = S0 + C, *V0 = sc + SCM, *V1 = V0 + C;
-                double term = 0.0;
-                for (int i2 = gl; i2 < N; i2 += kGS) {
-                    const int nr = s_nrem[i2];
-                    const double tq[3] = {S0[2 * i2], S0[2 * i2 + 1], S1[2 * i2] + S1[2 * i2 + 1]}, tp[3] = {V0[2 * i2], V0[2 * i2 + 1], V1[2 * i2] + V1[2 * i2 + 1]};
-                    for (int u = 0; u < nr; ++u) {
-                        double sq = 0.0;
-                        for (int v = 0; v < nr; ++v) sq += sGs[i2 * 9 + u * 3 + v] * tq[v];
-                        term += tp[u] * sq;
-                    }
-                }
-                al_mr = sc[SC_PQ] - group_sum(term);
+                al_mr = minres_alpha(scal + q.f * SB);                       // (batch: bitwise the value recorded in SC_ALPHA above)
+                if (!BATCH && rnd == 0 && tid == 0) { scal[SC_ALPHA] = al_mr; if (b == 0) a.alpha[0] = al_mr; }
             }
             if (act) {
                 const double *sc = scal + q.f * SB;
@@ -847,9 +867,8 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                     const double *S0 = sc + SC_HEAD, *S1 = sc + SC_HEAD + C;
                     const double tq[3] = {S0[2 * q.w], S0[2 * q.w + 1], S1[2 * q.w] + S1[2 * q.w + 1]};
                     const int nr = s_nrem[q.w];
-                    const double *Gw = sGs + q.w * 9;
-                    double d0 = 0.0, d2 = 0.0;
-                    for (int v = 0; v < nr; ++v) { d0 += Gw[q.comp * 3 + v] * tq[v]; d2 += Gw[6 + v] * tq[v]; }
+                    double d0, d2;
+                    modal_coef(sGs + q.w * 9, tq, nr, q.comp, d0, d2);
                     c0 = (q.comp < nr) ? (T)d0 : (T)0;
                     c2 = (2 < nr) ? (T)d2 : (T)0;
                 }
@@ -928,56 +947,60 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                         const double *V0 = sc + SCM, *V1 = V0 + C;
                         const double tp[3] = {V0[2 * q.w], V0[2 * q.w + 1], V1[2 * q.w] + V1[2 * q.w + 1]};
                         const int nr = s_nrem[q.w];
-                        const double *Gw = sGs + q.w * 9;
-                        double d0 = 0.0, d2 = 0.0;
-                        for (int v = 0; v < nr; ++v) { d0 += Gw[q.comp * 3 + v] * tp[v]; d2 += Gw[6 + v] * tp[v]; }
+                        double d0, d2;
+                        modal_coef(sGs + q.w * 9, tp, nr, q.comp, d0, d2);
                         cv0 = (q.comp < nr) ? (T)d0 : (T)0;
                         cv2 = (2 < nr) ? (T)d2 : (T)0;
                     }
                     constexpr int NX = (P / 2 + kGS) / kGS;              // columns per lane
-                    T vo_[NX][2], vc_[NX][2], w1_[NX][2], w2_[NX][2], xv_[NX][2];        // every load is issued before the first store
+                    constexpr int NH = (NX + 1) / 2;                     // two halves (five vectors: all columns at once spill);
+                                                                         // every load of a half is issued before its first store
 #pragma unroll
-                    for (int m = 0; m < NX; ++m) {
-                        const int xp = gl + m * kGS;
+                    for (int h0 = 0; h0 < NX; h0 += NH) {
+                        T vo_[NH][2], vc_[NH][2], w1_[NH][2], w2_[NH][2], xv_[NH][2];
 #pragma unroll
-                        for (int row = 0; row < 2; ++row) {
-                            vo_[m][row] = vc_[m][row] = w1_[m][row] = w2_[m][row] = xv_[m][row] = (T)0;
-                            if (xp < n && ((vm >> (row * 16 + m)) & 1u)) {
-                                const int idx = row * n + xp;
-                                if (!first) vo_[m][row] = uvo[idx];
-                                vc_[m][row] = uvc[idx];
-                                if (pon) { w1_[m][row] = uw1[idx]; w2_[m][row] = uw2[idx]; xv_[m][row] = ux[idx]; }
-                            }
-                        }
-                    }
-#pragma unroll
-                    for (int m = 0; m < NX; ++m) {
-                        const int xp = gl + m * kGS;
-                        if (xp < n) {
-                            const C2 z = bufA[xp];
-                            T nr[2] = {(T)0, (T)0};
+                        for (int mm = 0; mm < NH; ++mm) {
+                            const int m = h0 + mm, xp = gl + m * kGS;
 #pragma unroll
                             for (int row = 0; row < 2; ++row) {
-                                if ((vm >> (row * 16 + m)) & 1u) {
+                                vo_[mm][row] = vc_[mm][row] = w1_[mm][row] = w2_[mm][row] = xv_[mm][row] = (T)0;
+                                if (m < NX && xp < n && ((vm >> (row * 16 + m)) & 1u)) {
                                     const int idx = row * n + xp;
-                                    const T coord = ((q.comp ? (T)(q.y0 + row) : (T)xp) - half_n) * dd;
-                                    const T vo = vo_[m][row];
-                                    if (pon) {
-                                        const T w = (vo - peps * w2_[m][row] - pdelta * w1_[m][row]) * pinvg;
-                                        ux[idx] = xv_[m][row] + pphi * w;
-                                        uw2[idx] = w1_[m][row]; uw1[idx] = w;
-                                    }
-                                    if (!frozen) {
-                                        const T vp = vc_[m][row] * ib - (cv0 + cv2 * coord);
-                                        const T qp = (row ? -z.y : z.x) - (c0 + c2 * coord);
-                                        const T uv = qp - alm * vp - betak * vo;
-                                        uvo[idx] = vp; uvc[idx] = uv;
-                                        rr += (double)uv * (double)uv;
-                                        nr[row] = uv;
-                                    }
+                                    if (!first) vo_[mm][row] = uvo[idx];
+                                    vc_[mm][row] = uvc[idx];
+                                    if (pon) { w1_[mm][row] = uw1[idx]; w2_[mm][row] = uw2[idx]; xv_[mm][row] = ux[idx]; }
                                 }
                             }
-                            bufA[xp] = mk<T>(nr[0], nr[1]);
+                        }
+#pragma unroll
+                        for (int mm = 0; mm < NH; ++mm) {
+                            const int m = h0 + mm, xp = gl + m * kGS;
+                            if (m < NX && xp < n) {
+                                const C2 z = bufA[xp];
+                                T nr[2] = {(T)0, (T)0};
+#pragma unroll
+                                for (int row = 0; row < 2; ++row) {
+                                    if ((vm >> (row * 16 + m)) & 1u) {
+                                        const int idx = row * n + xp;
+                                        const T coord = ((q.comp ? (T)(q.y0 + row) : (T)xp) - half_n) * dd;
+                                        const T vo = vo_[mm][row];
+                                        if (pon) {
+                                            const T w = (vo - peps * w2_[mm][row] - pdelta * w1_[mm][row]) * pinvg;
+                                            ux[idx] = xv_[mm][row] + pphi * w;
+                                            uw2[idx] = w1_[mm][row]; uw1[idx] = w;
+                                        }
+                                        if (!frozen) {
+                                            const T vp = vc_[mm][row] * ib - (cv0 + cv2 * coord);
+                                            const T qp = (row ? -z.y : z.x) - (c0 + c2 * coord);
+                                            const T uv = qp - alm * vp - betak * vo;
+                                            uvo[idx] = vp; uvc[idx] = uv;
+                                            rr += (double)uv * (double)uv;
+                                            nr[row] = uv;
+                                        }
+                                    }
+                                }
+                                bufA[xp] = mk<T>(nr[0], nr[1]);
+                            }
                         }
                     }
                 };

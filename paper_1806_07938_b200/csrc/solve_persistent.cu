@@ -286,10 +286,10 @@ int cg_step_persistent(tomo_plan *pl, float *x, float *r, float *p, double *scal
     return state_store(pl, st, x, r, p);
 }
 
-// Measurement aid (tomo_time_phases): one instrumented persistent solve from the state the last solve left
-// (PM_STATE), thread 0 of every CTA stamps clock64 at the phase boundaries; returns, per segment, the mean over
+// Measurement aid (tomo_time_phases): one instrumented persistent solve -- CG from the state the last solve left
+// (PM_STATE), MINRES from a cold start on the projected slopes the last solve left in the plan -- thread 0 of every CTA stamps clock64 at the phase boundaries; returns, per segment, the mean over
 // iterations of the MAXIMUM over CTAs (work segments) or the MINIMUM over CTAs (barrier waits = pure latency).
-int time_phases_persistent(tomo_plan *pl, int F, int n_iter, float *us_out, cudaStream_t st) {
+int time_phases_persistent(tomo_plan *pl, int F, int n_iter, int minres, float *us_out, cudaStream_t st) {
     int rc;
     if ((rc = persist_prepare(pl))) return rc;
     PersistState *ps = (PersistState *)pl->persist;
@@ -298,7 +298,9 @@ int time_phases_persistent(tomo_plan *pl, int F, int n_iter, float *us_out, cuda
     const size_t cnt = (size_t)G * n_iter * PT_N;
     PCK(cudaMalloc(&d_dbg, cnt * sizeof(long long)));
     PCK(cudaMemsetAsync(d_dbg, 0, cnt * sizeof(long long), st));
-    rc = persist_dispatch(pl, st, F, n_iter, PM_STATE, 0, nullptr, nullptr, nullptr, d_dbg);
+    if (minres && pl->elem != 4) { cudaFree(d_dbg); set_error("tomo_time_phases: MINRES is instrumented for TOMO_F32 only"); return TOMO_EUNSUPPORTED; }
+    rc = minres ? persist_dispatch(pl, st, F, n_iter, PM_COLD, 0, (const float *)pl->d_b, nullptr, nullptr, d_dbg, METHOD_MINRES)
+                : persist_dispatch(pl, st, F, n_iter, PM_STATE, 0, nullptr, nullptr, nullptr, d_dbg);
     std::vector<long long> h(cnt);
     cudaError_t e = cudaStreamSynchronize(st);
     if (!rc && e == cudaSuccess) e = cudaMemcpy(h.data(), d_dbg, cnt * sizeof(long long), cudaMemcpyDeviceToHost);

@@ -758,7 +758,7 @@ static int check_ready(tomo_plan *pl) {
 namespace tomo {
 int solve_persistent(tomo_plan *pl, const float *slopes, float *out, int F, int n_iter, const float *x0, cudaStream_t st);
 int cg_step_persistent(tomo_plan *pl, float *x, float *r, float *p, double *scal, cudaStream_t st);
-int time_phases_persistent(tomo_plan *pl, int F, int n_iter, float *us_out, cudaStream_t st);
+int time_phases_persistent(tomo_plan *pl, int F, int n_iter, int minres, float *us_out, cudaStream_t st);
 int time_solver_persistent(tomo_plan *pl, const float *slopes, int F, int n_iter, int reps, int minres, float *ms_out, cudaStream_t st);
 
 // A7-A8 from the CG solution held in d_x -> d_out (used by the persistent solver)
@@ -841,11 +841,11 @@ extern "C" int tomo_time_kernels(tomo_plan *pl, int n_frames, int n_iter, float 
     return DISPATCH(pl, time_kernels(pl, n_frames, n_iter, ms_out, (cudaStream_t)cuda_stream));
 }
 
-extern "C" int tomo_time_phases(tomo_plan *pl, int n_frames, int n_iter, float *us_out, void *cuda_stream) {
+extern "C" int tomo_time_phases(tomo_plan *pl, int n_frames, int n_iter, int minres, float *us_out, void *cuda_stream) {
     int rc = check_ready(pl);
     if (rc) return rc;
     if (!us_out || n_frames < 1 || n_frames > pl->F || n_iter < 1 || n_iter >= pl->hist_cap) { set_error("bad arguments"); return TOMO_EINVAL; }
-    return time_phases_persistent(pl, n_frames, n_iter, us_out, (cudaStream_t)cuda_stream);
+    return time_phases_persistent(pl, n_frames, n_iter, minres, us_out, (cudaStream_t)cuda_stream);
 }
 
 extern "C" int tomo_time_solver(tomo_plan *pl, const float *slopes, int n_frames, int n_iter, int reps, int minres, float *ms_out,

@@ -93,7 +93,7 @@ def load(build_if_missing: bool = True):
     lib.tomo_cg_step.argtypes = [vp, fp, fp, fp, vp, vp]
     lib.tomo_get_zeta.argtypes = [vp, fp, C.c_int, vp]
     lib.tomo_time_kernels.argtypes = [vp, C.c_int, C.c_int, C.POINTER(C.c_float), vp]
-    lib.tomo_time_phases.argtypes = [vp, C.c_int, C.c_int, C.POINTER(C.c_float), vp]
+    lib.tomo_time_phases.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_float), vp]
     lib.tomo_time_solver.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_float), vp]
     lib.tomo_get_sizes.argtypes = [vp, ip, ip, ip, ip, ip, ip, ip]
     lib.tomo_get_valid_index.argtypes = [vp, ip, ip]
@@ -353,9 +353,9 @@ class TomoPlan:
         _check(self.lib.tomo_time_kernels(self._h, n_frames, n_iter, ms, _stream_handle(stream)))
         return dict(zip(("rows_fwd", "cols", "rows_inv", "update"), [float(v) for v in ms]))
 
-    def time_phases(self, n_frames: int, n_iter: int, stream=None):
+    def time_phases(self, n_frames: int, n_iter: int, stream=None, minres: bool = False):
         us = (C.c_float * 10)()
-        _check(self.lib.tomo_time_phases(self._h, n_frames, n_iter, us, _stream_handle(stream)))
+        _check(self.lib.tomo_time_phases(self._h, n_frames, n_iter, 1 if minres else 0, us, _stream_handle(stream)))
         return dict(zip(("iteration", "rho_beta", "slab_update", "slab_fft_fwd", "slab_mac", "slab_fft_inv", "barrier_b", "alpha_modes",
                          "rows", "barrier_a"),
                         [float(v) for v in us]))
