@@ -179,7 +179,9 @@ int tomo_time_kernels(tomo_plan *plan, int n_frames, int n_iter, float *ms_out, 
  * segments are the maximum over CTAs, barrier segments the minimum over CTAs (= pure latency):
  * [0] whole iteration (CTA 0), [1] rho/beta scalars, [2] p~ update, [3] forward y-FFT, [4] block product,
  * [5] inverse y-FFT + T2 write, [6] grid barrier B, [7] alpha/mode scalars (+ first inverse x-FFT), [8] row phase,
- * [9] grid barrier A.  The state of the last solve is overwritten. */
+ * [9] grid barrier A.  The state of the last solve is overwritten.  If the environment variable TOMO_STAMP_DUMP names a
+ * writable file, the raw per-CTA timeline (mean over iterations of every stamp, microseconds from the iteration start, one
+ * line per CTA) is also written there; the library reads no other environment variable. */
 int tomo_time_phases(tomo_plan *plan, int n_frames, int n_iter, int minres, float *us_out, void *cuda_stream);
 
 /* Measurement aid (bench.py "roofline" with the persistent solver): `reps` launches of the persistent kernel alone

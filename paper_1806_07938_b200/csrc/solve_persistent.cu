@@ -156,13 +156,12 @@ static int persist_prepare(tomo_plan *pl) {
     off += (size_t)std::max(maxu, 1) * sizeof(UnitRec);
     off = align16(off);
     const size_t spec_bytes = (size_t)m.n_pair * m.P * 2 * SE, vec_bytes = (size_t)maxu * 6 * m.n * E, vec_bytes_mr = (size_t)maxu * 10 * m.n * E;
-    const char *no_pin = getenv("TOMO_NO_SPEC_SMEM"), *no_vec = getenv("TOMO_NO_VEC_SMEM");
     // the spectra slice has priority for the shared memory that is left, then the CG vectors of the CTA's row units
     ps->off_spec = (int)off;
-    ps->spec_smem = (off + spec_bytes <= (size_t)max_smem) && !(no_pin && no_pin[0] == '1');
+    ps->spec_smem = off + spec_bytes <= (size_t)max_smem;
     if (ps->spec_smem) off = align16(off + spec_bytes);
     ps->off_vec = (int)off;
-    ps->vec_smem = (off + vec_bytes <= (size_t)max_smem) && !(no_vec && no_vec[0] == '1');
+    ps->vec_smem = off + vec_bytes <= (size_t)max_smem;
     ps->vec_smem_mr = ps->vec_smem && (off + vec_bytes_mr <= (size_t)max_smem);      // MINRES keeps five row vectors per unit
     if (ps->vec_smem) off = align16(off + (ps->vec_smem_mr ? vec_bytes_mr : vec_bytes));
     if (off > (size_t)max_smem) { delete ps; set_error("persistent solver: problem too large for shared memory"); return TOMO_EUNSUPPORTED; }

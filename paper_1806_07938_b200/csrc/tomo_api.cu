@@ -289,6 +289,17 @@ static inline void prof_mark(tomo_plan *pl, cudaStream_t st) {
     pl->prof->push_back(e);
 }
 
+// Instantiated solve graphs are kept per (frames, iterations, flags).  The cache is bounded: a caller that sweeps many
+// iteration counts on one plan would otherwise keep every graph alive; at the cap all are destroyed and rebuilt on demand
+// (a graph still in flight on a stream finishes first: cudaGraphExecDestroy defers the release).
+static const size_t kMaxGraphs = 32;
+static inline void graph_cache_make_room(tomo_plan *pl) {
+    if (pl->graphs.size() < kMaxGraphs) return;
+    for (auto &kv : pl->graphs) cudaGraphExecDestroy(kv.second);
+    pl->graphs.clear();
+    pl->graph_launches.clear();
+}
+
 template <typename T, typename S> struct Ops {
     typedef typename cx_of<T>::type C2;
     typedef typename cx_of<S>::type S2;
@@ -447,14 +458,12 @@ template <typename T, typename S> struct Ops {
             pl->launches_last += 3;
             n_part0 = pl->upd_blocks;
         }
-        const char *no_graph = getenv("TOMO_NO_GRAPH");
-        if (no_graph && no_graph[0] == '1') {
-            if ((rc = enqueue_loop(pl, st, F, n_iter, n_part0, with_cos))) return rc;
-        } else {
+        {
             const auto key = std::make_tuple(F, n_iter, (x0 ? 1 : 0) + (with_cos ? 2 : 0));
             auto it = pl->graphs.find(key);
             const int before = pl->launches_last;
             if (it == pl->graphs.end()) {
+                graph_cache_make_room(pl);
                 cudaStream_t cs;
                 CK(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
                 CK(cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal));
@@ -520,12 +529,12 @@ template <typename T, typename S> struct Ops {
         const HostModel &m = pl->m;
         int rc;
         if ((rc = prepare(pl))) return rc;
-        if (!pl->d_mstate) {
+        {   // allocated on the first MINRES solve; each buffer on its own check, so a retry after a failure allocates none twice
             const size_t vec = (size_t)pl->F * m.C * m.nv * pl->elem;
-            if ((rc = dev_alloc_bytes(pl, &pl->d_vold, vec))) return rc;
-            if ((rc = dev_alloc_bytes(pl, &pl->d_w1, vec))) return rc;
-            if ((rc = dev_alloc_bytes(pl, &pl->d_w2, vec))) return rc;
-            if ((rc = dev_alloc<double>(pl, &pl->d_mstate, (size_t)2 * pl->F * MS_N))) return rc;
+            if (!pl->d_vold && (rc = dev_alloc_bytes(pl, &pl->d_vold, vec))) return rc;
+            if (!pl->d_w1 && (rc = dev_alloc_bytes(pl, &pl->d_w1, vec))) return rc;
+            if (!pl->d_w2 && (rc = dev_alloc_bytes(pl, &pl->d_w2, vec))) return rc;
+            if (!pl->d_mstate && (rc = dev_alloc<double>(pl, &pl->d_mstate, (size_t)2 * pl->F * MS_N))) return rc;
         }
         pl->launches_last = 0;
         const bool with_cos = pl->has_cos && out != nullptr;
@@ -553,6 +562,7 @@ template <typename T, typename S> struct Ops {
         auto it = pl->graphs.find(key);
         const int before = pl->launches_last;
         if (it == pl->graphs.end()) {
+            graph_cache_make_room(pl);
             cudaStream_t cs;
             CK(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
             CK(cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal));
@@ -662,11 +672,11 @@ template <typename T, typename S> struct Ops {
     static int project_from_x(tomo_plan *pl, cudaStream_t st, int F) {
         int rc;
         if ((rc = prepare(pl))) return rc;
-        const char *no_graph = getenv("TOMO_NO_GRAPH");
-        if (!(no_graph && no_graph[0] == '1')) {
+        {
             const auto key = std::make_tuple(F, -1, 8);
             auto it = pl->graphs.find(key);
             if (it == pl->graphs.end()) {
+                graph_cache_make_room(pl);
                 const int before = pl->launches_last;
                 cudaStream_t cs;
                 CK(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
@@ -689,7 +699,6 @@ template <typename T, typename S> struct Ops {
             CK(cudaGraphLaunch(it->second, st));
             return TOMO_OK;
         }
-        return project_from_x_enqueue(pl, st, F);
     }
 
     static int project_from_x_enqueue(tomo_plan *pl, cudaStream_t st, int F) {
@@ -905,8 +914,11 @@ extern "C" int tomo_measure_device(long long l2_bytes, int reps, float *out, voi
     float4 *buf = nullptr;
     float *sink = nullptr;
     CK(cudaMalloc(&buf, n4 * 16));
-    CK(cudaMalloc(&sink, 16));
-    CK(cudaMemsetAsync(buf, 0, n4 * 16, st));
+    if (cudaMalloc(&sink, 16) != cudaSuccess || cudaMemsetAsync(buf, 0, n4 * 16, st) != cudaSuccess) {
+        set_error(std::string("tomo_measure_device: ") + cudaGetErrorString(cudaGetLastError()));
+        cudaFree(buf); cudaFree(sink);
+        return TOMO_ECUDA;
+    }
     cudaEvent_t e0, e1;
     cudaEventCreate(&e0); cudaEventCreate(&e1);
     const int sweeps = 20;
