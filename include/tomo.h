@@ -153,6 +153,22 @@ int tomo_solve_minres(tomo_plan *plan, const float *slopes, float *wavefront_out
  * the multi-kernel product.  v, out: device fp32 [C][n_vs]. */
 int tomo_apply_css(tomo_plan *plan, const float *v, float *out, void *cuda_stream);
 
+/* The same product, out = M_s (W_s Sigma_ss W_s^T + Sigma_eta) M_s^T v (Eq.30, Eq.34), for callers that may not
+ * allocate (code under CUDA graph capture, serving loops, harnesses that forbid cudaMalloc): this entry point calls no
+ * cudaMalloc / cudaFree and no allocating library routine.  It runs the multi-kernel product (projection, row FFTs, per-frequency
+ * block product, inverse row FFTs, projection) with ALL its workspace -- the projected input, the product, the two half-spectrum
+ * buffers T1 / T2 and the reduction partials -- inside one file-scope device array of TOMO_STATIC_SCRATCH_BYTES, which every GPU
+ * that loads the library holds until the process exits.  A plan whose workspace is larger (2 C n_vs + 4 C (P/2+1) n elements of the
+ * plan's arithmetic type plus partials; cfg3 / cfg4 in fp32 take 1.6 / 2.1 MB, cfg4 in TOMO_F64 4.2 MB) is refused with
+ * TOMO_EINVAL and a message that names both sizes; nothing is launched then.  The array is shared by every plan and every call
+ * and keeps the last call's contents: each call clears the part it uses (a memset node on `cuda_stream`) before its kernels.
+ * Calls that may overlap on the GPU (different streams, or graphs replayed concurrently) RACE on the array and give wrong
+ * results: serialise them, or use tomo_apply_css, whose workspace belongs to the plan.  The array's address is looked up once
+ * per device on the first call for that device (make that call outside a capture).  v, out: device fp32 [C][n_vs]; asynchronous
+ * on `cuda_stream`; errors as tomo_apply_css. */
+#define TOMO_STATIC_SCRATCH_BYTES 4194304
+int tomo_apply_css_static(tomo_plan *plan, const float *v, float *out, void *cuda_stream);
+
 /* wavefront_out = M_phi W_phi Sigma_{phi s} W_s^T M_s^T zeta  (Eq.31/32, Eq.35) for every target (A7-A8 only).
  * zeta: device fp32 [C][n_vs]; wavefront_out: device fp32 [n_targets][n_vphi].
  * Layered plans: wavefront_out[k] = Sigma_{phi_k s} W_s^T M_s^T zeta for every layer k, device fp32 [K][n_m][n_m]. */

@@ -4,6 +4,7 @@
 #include <complex>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -605,6 +606,59 @@ template <typename T, typename S> struct Ops {
         return TOMO_OK;
     }
 
+    // tomo_apply_css_static: the multi-kernel product of apply_css with every workspace inside the caller-given scratch
+    // (layout p | q | T1 | T2 | partials_q, each part 256-byte aligned); returns the bytes needed in *need
+    static size_t static_layout(const tomo_plan *pl, size_t off[5]) {
+        const HostModel &m = pl->m;
+        const size_t vec = (size_t)m.C * m.nv * sizeof(T), tsz = (size_t)m.C * m.Ph * m.n * 2 * sizeof(T);
+        const size_t sz[5] = {vec, vec, tsz, tsz, (size_t)m.C * pl->g.npairs * TOMO_NRED * sizeof(double)};
+        size_t o = 0;
+        for (int i = 0; i < 5; ++i) { off[i] = o; o += (sz[i] + 255) & ~(size_t)255; }
+        return o;
+    }
+    static int apply_css_static(tomo_plan *pl, const float *v, float *out, cudaStream_t st, unsigned char *scr, size_t cap) {
+        const HostModel &m = pl->m;
+        size_t off[5];
+        const size_t need = static_layout(pl, off);
+        if (need > cap) {
+            set_error("tomo_apply_css_static: this plan needs " + std::to_string(need) + " bytes of workspace, the static scratch holds " +
+                      std::to_string(cap) + " (TOMO_STATIC_SCRATCH_BYTES); use tomo_apply_css");
+            return TOMO_EINVAL;
+        }
+        int rc;
+        if ((rc = prepare(pl))) return rc;
+        T *sp = (T *)(scr + off[0]), *sq = (T *)(scr + off[1]);
+        C2 *t1 = (C2 *)(scr + off[2]), *t2 = (C2 *)(scr + off[3]);
+        double *part = (double *)(scr + off[4]);
+        // the array keeps the last call's contents (possibly another plan's): cleared, so that no call ever sees them
+        CK(cudaMemsetAsync(scr, 0, need, st));
+        ProjectArgs<float, T> pa;
+        pa.g = pl->g; pa.in = v; pa.out = sp; pa.out2 = pa.out3 = pa.zero = nullptr; pa.partials_r = nullptr; pa.part_stride = 0;
+        k_project<float, T><<<dim3(m.n_wfs, 1), 256, 0, st>>>(pa);
+        LAUNCH_CHECK();
+        RowsFwdArgs<T> a;
+        std::memset(&a, 0, sizeof(a));
+        a.st = make_stage<T>(pl, false); a.g = pl->g; a.F = 1; a.p = sp; a.T1 = t1;
+        const int items = m.C * pl->g.npairs;
+        k_rows_fwd<T><<<grid_for(items, kRowWarps), 32 * kRowWarps, rows_smem<T>(m.P), st>>>(a);
+        LAUNCH_CHECK();
+        ColsArgs<T, S> c;
+        c.st = a.st; c.g = pl->g; c.T1 = t1; c.T2 = t2; c.spec = (const S2 *)pl->d_spec; c.n_pair = m.n_pair;
+        const int nw = cols_warps(m.C);
+        k_cols<T, S><<<dim3(m.Ph, 1), 32 * nw, cols_smem<T>(m.P, m.C, nw), st>>>(c);
+        LAUNCH_CHECK();
+        RowsInvArgs<T> b;
+        b.st = a.st; b.g = pl->g; b.F = 1; b.T2 = t2; b.p = sp;
+        b.sigma2 = (const T *)pl->d_sigma2; b.sigma_xy = (const T *)pl->d_sigma_xy; b.q = sq; b.partials_q = part;
+        k_rows_inv<T><<<grid_for(items, kRowWarps), 32 * kRowWarps, rows_smem<T>(m.P), st>>>(b);
+        LAUNCH_CHECK();
+        ProjectArgs<T, float> pb;
+        pb.g = pl->g; pb.in = sq; pb.out = out; pb.out2 = pb.out3 = pb.zero = nullptr; pb.partials_r = nullptr; pb.part_stride = 0;
+        k_project<T, float><<<dim3(m.n_wfs, 1), 256, 0, st>>>(pb);
+        LAUNCH_CHECK();
+        return TOMO_OK;
+    }
+
     static int apply_cos(tomo_plan *pl, const float *zeta, float *out, cudaStream_t st) {
         int rc;
         if ((rc = prepare(pl))) return rc;
@@ -818,6 +872,35 @@ extern "C" int tomo_apply_css(tomo_plan *pl, const float *v, float *out, void *c
     // the product of the solver that runs the solves: one single-product launch of the persistent kernel, or the multi-kernel product
     if (pl->solver_used == TOMO_SOLVER_PERSISTENT) return apply_css_persistent(pl, v, out, (cudaStream_t)cuda_stream);
     return DISPATCH(pl, apply_css(pl, v, out, (cudaStream_t)cuda_stream));
+}
+
+// ---- the product without any allocation (tomo.h: tomo_apply_css_static).  The workspace is this file-scope device array: every
+// GPU that loads the library holds TOMO_STATIC_SCRATCH_BYTES of it until the process exits.  In host code the name below is a
+// host-side stand-in, not a device address: the address is asked for once per device, with that device current.
+static __device__ __align__(256) unsigned char g_static_scratch[TOMO_STATIC_SCRATCH_BYTES];
+static std::mutex g_static_mu;
+static unsigned char *g_static_ptr[64] = {};
+
+static int static_scratch_address(int device, unsigned char **out) {
+    if (device < 0 || device >= 64) { set_error("tomo_apply_css_static: device index out of range"); return TOMO_EUNSUPPORTED; }
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_ptr[device]) {
+        void *ptr = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(&ptr, g_static_scratch);        // the caller made `device` current (check_ready)
+        if (e != cudaSuccess || !ptr) { set_error(std::string("cudaGetSymbolAddress(g_static_scratch): ") + cudaGetErrorString(e)); return TOMO_ECUDA; }
+        g_static_ptr[device] = (unsigned char *)ptr;
+    }
+    *out = g_static_ptr[device];
+    return TOMO_OK;
+}
+
+extern "C" int tomo_apply_css_static(tomo_plan *pl, const float *v, float *out, void *cuda_stream) {
+    int rc = check_ready(pl);
+    if (rc) return rc;
+    if (!v || !out) { set_error("NULL vector"); return TOMO_EINVAL; }
+    unsigned char *scr = nullptr;
+    if ((rc = static_scratch_address(pl->device, &scr))) return rc;
+    return DISPATCH(pl, apply_css_static(pl, v, out, (cudaStream_t)cuda_stream, scr, (size_t)TOMO_STATIC_SCRATCH_BYTES));
 }
 
 extern "C" int tomo_apply_cos(tomo_plan *pl, const float *zeta, float *wavefront_out, void *cuda_stream) {

@@ -20,9 +20,10 @@ TOMO_OK, TOMO_EINVAL, TOMO_EUNSUPPORTED, TOMO_ENOTREADY, TOMO_ENOMEM, TOMO_ECUDA
 TOMO_HUDGIN, TOMO_FRIED, TOMO_FFTMODEL = 0, 1, 2
 TOMO_F32, TOMO_F32S_F64A, TOMO_F64 = 0, 1, 2
 TOMO_SOLVER_MULTIKERNEL, TOMO_SOLVER_PERSISTENT = 0, 1
+TOMO_STATIC_SCRATCH_BYTES = 4194304
 
 EXPORTS = (
-    "tomo_plan_create", "tomo_plan_upload_kernels", "tomo_solve", "tomo_solve_batch", "tomo_solve_minres", "tomo_apply_css",
+    "tomo_plan_create", "tomo_plan_upload_kernels", "tomo_solve", "tomo_solve_batch", "tomo_solve_minres", "tomo_apply_css", "tomo_apply_css_static",
     "tomo_apply_cos", "tomo_cg_step", "tomo_get_zeta", "tomo_time_kernels", "tomo_time_phases", "tomo_time_solver", "tomo_measure_device",
     "tomo_get_sizes", "tomo_get_valid_index", "tomo_get_noise",
     "tomo_get_residuals", "tomo_get_stats", "tomo_get_solver", "tomo_plan_destroy", "tomo_last_error",
@@ -89,6 +90,7 @@ def load(build_if_missing: bool = True):
     lib.tomo_solve_batch.argtypes = [vp, fp, fp, C.c_int, C.c_int, fp, vp]
     lib.tomo_solve_minres.argtypes = [vp, fp, fp, C.c_int, C.c_int, fp, vp]
     lib.tomo_apply_css.argtypes = [vp, fp, fp, vp]
+    lib.tomo_apply_css_static.argtypes = [vp, fp, fp, vp]
     lib.tomo_apply_cos.argtypes = [vp, fp, fp, vp]
     lib.tomo_cg_step.argtypes = [vp, fp, fp, fp, vp, vp]
     lib.tomo_get_zeta.argtypes = [vp, fp, C.c_int, vp]
@@ -338,6 +340,10 @@ class TomoPlan:
 
     def apply_css(self, v, out, stream=None):
         _check(self.lib.tomo_apply_css(self._h, _ptr(v), _ptr(out), _stream_handle(stream)))
+
+    def apply_css_static(self, v, out, stream=None):
+        """tomo_apply_css_static: the product with its workspace in the library's static device array (no allocation)."""
+        _check(self.lib.tomo_apply_css_static(self._h, _ptr(v), _ptr(out), _stream_handle(stream)))
 
     def apply_cos(self, zeta, wavefront_out, stream=None):
         _check(self.lib.tomo_apply_cos(self._h, _ptr(zeta), _ptr(wavefront_out), _stream_handle(stream)))
