@@ -215,14 +215,14 @@ def kernel_source_hash():
     return h.hexdigest()[:16]
 
 
-def stored_traffic(workload, batch, precision):
+def stored_traffic(workload, batch, precision, method="cg"):
     """dram__bytes_read.sum + dram__bytes_write.sum of one k_persistent launch from the committed ncu capture
-    (profiles/r2_traffic.json), or None when there is none for this (workload, batch, precision) or the kernel has changed since."""
+    (profiles/r2_traffic.json), or None when there is none for this (workload, batch, precision, method) or the kernel has changed since."""
     p = os.path.join(ROOT, "profiles", "r2_traffic.json")
     if not os.path.exists(p):
         return None
     for e in json.load(open(p)).get("entries", []):
-        if (e["workload"], e["batch"], e["precision"]) == (workload, batch, precision) and e["kernel_source_hash"] == kernel_source_hash():
+        if (e["workload"], e["batch"], e["precision"], e.get("method", "cg")) == (workload, batch, precision, method) and e["kernel_source_hash"] == kernel_source_hash():
             return e["dram_bytes_per_launch"]
     return None
 
@@ -362,7 +362,7 @@ def main():
         roof = {"kernel": "k_persistent", "bound": "hbm", "achieved": ach, "peak": hbm, "unit": "GB/s", "frac": ach / hbm,
                 # dram__bytes_read.sum + dram__bytes_write.sum of one launch from the committed ncu capture of THIS kernel source
                 # (profiles/r2_traffic.json, keyed by workload, batch, precision and source hash), else null
-                "traffic": stored_traffic(cfg.name, B, args.precision), "kernel_source_hash": kernel_source_hash(),
+                "traffic": stored_traffic(cfg.name, B, args.precision, args.method), "kernel_source_hash": kernel_source_hash(),
                 "peak_source": how, "algorithmic_bytes_per_launch": kb,
                 "ms_per_launch": k_ms, "ms_per_launch_n_iter0": k_ms0,
                 "us_per_iteration_in_kernel": (k_ms - k_ms0) / n_iter * 1e3,
