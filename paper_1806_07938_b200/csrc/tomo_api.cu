@@ -6,6 +6,7 @@
 #include <cstring>
 #include <mutex>
 #include <string>
+#include <type_traits>
 #include <vector>
 
 #include "tomo.h"
@@ -317,7 +318,31 @@ template <typename T, typename S> struct Ops {
         CK(cudaFuncSetAttribute(k_cos_rows_inv<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rs));
         CK(cudaFuncSetAttribute((k_cos_mac_inv<T, S>), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rs));
         CK(cudaFuncSetAttribute((k_cols<T, S>), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cs));
+        if constexpr (std::is_same<T, float>::value && std::is_same<S, float>::value) {
+            const int ns = cos_bulk_stages(pl);
+            if (ns > 0) {
+                const int sm = (int)cos_bulk_smem(m.C, m.P_os, ns);
+                switch (m.C) {
+                    case 4: CK(cudaFuncSetAttribute(k_cos_mac_bulk<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm)); break;
+                    case 6: CK(cudaFuncSetAttribute(k_cos_mac_bulk<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm)); break;
+                    case 8: CK(cudaFuncSetAttribute(k_cos_mac_bulk<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm)); break;
+                    case 12: CK(cudaFuncSetAttribute(k_cos_mac_bulk<12>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm)); break;
+                    default: CK(cudaFuncSetAttribute(k_cos_mac_bulk<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm)); break;
+                }
+            }
+        }
         return TOMO_OK;
+    }
+
+    // stages of the bulk-copy ring of k_cos_mac_bulk (two CTAs per SM), 0 = the kernel does not apply to this plan
+    static int cos_bulk_stages(const tomo_plan *pl) {
+        if (!(std::is_same<T, float>::value && std::is_same<S, float>::value)) return 0;
+        const HostModel &m = pl->m;
+        if (!pl->has_cos || m.P_os > kCosBulkThreads) return 0;
+        if (m.C != 4 && m.C != 6 && m.C != 8 && m.C != 12 && m.C != 16) return 0;
+        int ns = 0;
+        while (ns < kCosBulkMaxStages && cos_bulk_smem(m.C, m.P_os, ns + 1) <= (size_t)112 * 1024) ++ns;
+        return ns >= 2 ? ns : 0;
     }
 
     // W (Sigma_ss + Sigma_eta) W^T p -> q (modes not removed) + reduction partials; p optionally updated first
@@ -379,7 +404,22 @@ template <typename T, typename S> struct Ops {
             CosMacArgs<T, S> mm;
             mm.st = so; mm.g = pl->g; mm.F = Fn; mm.Zs = (const C2 *)pl->d_Zs; mm.spec = (const S2 *)pl->d_spec_os;
             mm.T2 = (C2 *)pl->d_T2os;
-            k_cos_mac_inv<T, S><<<grid_for(m.T * m.Kp * m.Ph_os, kRowWarps), 32 * kRowWarps, rs, st>>>(mm);
+            int ns = 0;
+            if (Fn == 1 && (ns = cos_bulk_stages(pl)) > 0) {       // one frame, fp32: the spectra stream through a bulk-copy ring
+                if constexpr (std::is_same<T, float>::value && std::is_same<S, float>::value) {
+                    const int grid = std::min(2 * 148, m.T * m.Kp * m.Ph_os);
+                    const size_t sm = cos_bulk_smem(m.C, m.P_os, ns);
+                    switch (m.C) {
+                        case 4: k_cos_mac_bulk<4><<<grid, kCosBulkThreads, sm, st>>>(mm, ns); break;
+                        case 6: k_cos_mac_bulk<6><<<grid, kCosBulkThreads, sm, st>>>(mm, ns); break;
+                        case 8: k_cos_mac_bulk<8><<<grid, kCosBulkThreads, sm, st>>>(mm, ns); break;
+                        case 12: k_cos_mac_bulk<12><<<grid, kCosBulkThreads, sm, st>>>(mm, ns); break;
+                        default: k_cos_mac_bulk<16><<<grid, kCosBulkThreads, sm, st>>>(mm, ns); break;
+                    }
+                }
+            } else {
+                k_cos_mac_inv<T, S><<<grid_for(m.T * m.Kp * m.Ph_os, kRowWarps), 32 * kRowWarps, rs, st>>>(mm);
+            }
             LAUNCH_CHECK();
             CosRowsArgs<T> r;
             r.st = so; r.g = pl->g; r.F = Fn; r.T2 = (const C2 *)pl->d_T2os; r.G = (T *)pl->d_G;

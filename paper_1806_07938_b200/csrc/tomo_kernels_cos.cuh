@@ -155,6 +155,15 @@ __global__ void __launch_bounds__(128) k_cos_cols_fwd(CosColsArgs<T> a) {
     }
 }
 
+// (ar, ai) += (sx + i sy)(zx + i zy) with the contraction written out: k_cos_mac_inv and k_cos_mac_bulk round identically, so a frame
+// of a batch (the former) equals its single-frame solve (the latter) bit for bit
+__device__ __forceinline__ void cmac_acc(float &ar, float &ai, float sx, float sy, float zx, float zy) {
+    ar = __fmaf_rn(sx, zx, ar); ar = __fmaf_rn(-sy, zy, ar); ai = __fmaf_rn(sx, zy, ai); ai = __fmaf_rn(sy, zx, ai);
+}
+__device__ __forceinline__ void cmac_acc(double &ar, double &ai, double sx, double sy, double zx, double zy) {
+    ar = __fma_rn(sx, zx, ar); ar = __fma_rn(-sy, zy, ar); ai = __fma_rn(sx, zy, ai); ai = __fma_rn(sy, zx, ai);
+}
+
 // per (target, layer, kx): g~(ky) = sum_c xi~'(c, ky) zeta~_c(ky) for every frame of the chunk (the spectra are
 // read from HBM once and reused from L1/L2 for the other frames), inverse FFT along y, keep rows y < n'.
 template <typename T, typename S> struct CosMacArgs {
@@ -188,8 +197,7 @@ __global__ void __launch_bounds__(128) k_cos_mac_inv(CosMacArgs<T, S> a) {
                 for (int c = 0; c < C; ++c) {
                     const S2 s = sp[(size_t)c * P + i];
                     const C2 z = zs[(size_t)c * P + i];
-                    ar += (T)s.x * z.x - (T)s.y * z.y;
-                    ai += (T)s.x * z.y + (T)s.y * z.x;
+                    cmac_acc(ar, ai, (T)s.x, (T)s.y, z.x, z.y);
                 }
                 A[i] = mk<T>(ar, ai);
             }
@@ -198,6 +206,112 @@ __global__ void __launch_bounds__(128) k_cos_mac_inv(CosMacArgs<T, S> a) {
             for (int i = lane; i < np; i += 32) dst[i] = Z[i];
             __syncwarp();
         }
+    }
+}
+
+// ---- bulk-copy variant of k_cos_mac_inv (one frame, fp32, P <= 256, C a compile-time constant).
+// The kernel above keeps the streamed spectra in flight through registers: 36 warps per SM, each waiting on its own loads
+// (long_scoreboard 64 % of the samples, 64 % of the HBM peak at cfg4).  Here the spectra of one (target, layer, k_x) item -- C P
+// complex64, contiguous in HBM -- arrive by ONE bulk copy (`cp.async.bulk`, completion on an mbarrier) into a ring of stages
+// shared by the whole CTA, so that the bytes in flight cost no registers and no warp has to wait for its own data:
+//   * a CTA owns a contiguous range of items in [k_x][target, layer] order; thread ky < P keeps zeta~_c(k_x, ky), c < C, in
+//     registers for as long as k_x stays the same;
+//   * per item: wait for its stage, every thread forms g~(ky) = sum_c xi~'(c, ky) zeta~_c(ky) from shared memory and writes it to
+//     one of NW small FFT buffers, the stage is refilled at once with the item NS ahead;
+//   * every NW items the NW warps run one inverse y-FFT each and store rows y < n' (same warp_fft, same order of operations as
+//     k_cos_mac_inv, see cmac_acc: the results are bitwise the same).
+static const int kCosBulkThreads = 256;
+static const int kCosBulkMaxStages = 8;
+
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t"
+        "}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned bytes, unsigned long long *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+// shared memory: ring[NS][CT P] | tw[P] | fb[NW][2][P] | full[NS]
+static inline size_t cos_bulk_smem(int C, int P, int NS) {
+    return ((size_t)NS * C * P + P + (size_t)(kCosBulkThreads / 32) * 2 * P) * 2 * sizeof(float) + (size_t)NS * 8;
+}
+
+template <int CT>
+__global__ void __launch_bounds__(kCosBulkThreads, 2) k_cos_mac_bulk(CosMacArgs<float, float> a, int NS) {
+    typedef float2 C2;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int P = a.st.P, Ph = a.st.Ph, np = a.g.n_p, TK = a.g.T * a.g.Kp;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    constexpr int NW = kCosBulkThreads / 32;
+    const size_t stage = (size_t)CT * P;
+    C2 *ring = reinterpret_cast<C2 *>(smem_raw);
+    C2 *tw = ring + (size_t)NS * stage;
+    C2 *fb = tw + P;
+    unsigned long long *full = reinterpret_cast<unsigned long long *>(fb + (size_t)NW * 2 * P);
+    const unsigned bytes = (unsigned)(stage * sizeof(C2));
+    // this CTA's items e in [e0, e1), e = kx TK + tk
+    const int total = Ph * TK, per = (total + gridDim.x - 1) / gridDim.x;
+    const int e0 = min(total, (int)blockIdx.x * per), e1 = min(total, e0 + per), n_my = e1 - e0;
+    auto src_of = [&](int e) { const int kx = e / TK, tk = e - kx * TK; return a.spec + ((size_t)tk * Ph + kx) * stage; };
+    if (tid == 0) {
+        for (int s = 0; s < NS; ++s) mbar_init(full + s, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    load_twiddles<float>(tw, a.st);
+    __syncthreads();
+    if (tid == 0)
+        for (int s = 0; s < NS && s < n_my; ++s) { mbar_expect_tx(full + s, bytes); bulk_g2s(ring + (size_t)s * stage, src_of(e0 + s), bytes, full + s); }
+    C2 z[CT];
+    int kx_cur = -1;
+#pragma unroll 1
+    for (int i = 0; i < n_my; ++i) {
+        const int e = e0 + i, kx = e / TK, tk = e - kx * TK, s = i % NS, j = i % NW;
+        if (kx != kx_cur) {
+            kx_cur = kx;
+            if (tid < P) {
+#pragma unroll
+                for (int c = 0; c < CT; ++c) z[c] = a.Zs[((size_t)kx * CT + c) * P + tid];
+            }
+        }
+        mbar_wait(full + s, (unsigned)((i / NS) & 1));
+        if (tid < P) {
+            const C2 *sp = ring + (size_t)s * stage + tid;
+            float ar = 0.f, ai = 0.f;
+#pragma unroll
+            for (int c = 0; c < CT; ++c) {
+                const C2 v = sp[(size_t)c * P];
+                cmac_acc(ar, ai, v.x, v.y, z[c].x, z[c].y);
+            }
+            fb[(size_t)j * 2 * P + tid] = make_float2(ar, ai);
+        }
+        __syncthreads();                                    // the stage has been read by everyone, fb[j] is complete
+        if (tid == 0 && i + NS < n_my) { mbar_expect_tx(full + s, bytes); bulk_g2s(ring + (size_t)s * stage, src_of(e + NS), bytes, full + s); }
+        if (j == NW - 1 || i == n_my - 1) {
+            if (warp <= j) {
+                const int ei = e - j + warp, kxi = ei / TK, tki = ei - kxi * TK;
+                C2 *A = fb + (size_t)warp * 2 * P;
+                C2 *Z = warp_fft<float, true>(A, A + P, a.st.fd, tw, lane);
+                C2 *dst = a.T2 + ((size_t)tki * Ph + kxi) * np;
+                for (int y = lane; y < np; y += 32) dst[y] = Z[y];
+            }
+            __syncthreads();                                // before the next group overwrites the FFT buffers
+        }
+        (void)tk;
     }
 }
 
