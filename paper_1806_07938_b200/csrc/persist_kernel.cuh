@@ -200,7 +200,7 @@ struct UnitRec { int f, c, j, s0, s1, s2, pad0, pad1; };   // row unit of a CTA:
 
 // ---- the rows [LO, HI) of the block product for one k_y, straight-line: every pair index and conjugation is a
 // compile-time constant, no branch between the rows (the loads of the next row overlap the FMAs of this one)
-template <typename T, typename S, int CT, int PP, int LO, int HI>
+template <typename T, typename S, int CT, int PP, int LO, int HI, bool MR = false>
 __device__ __forceinline__ void mac_rows(const typename cx_of<T>::type (&x)[CT], const typename cx_of<S>::type *sp, const T *s2c,
                                          typename cx_of<T>::type *Y, int LD, int ky, typename cx_of<T>::type m0,
                                          typename cx_of<T>::type m1, typename cx_of<T>::type m2, T *red_s, T *red_f,
@@ -230,17 +230,23 @@ __device__ __forceinline__ void mac_rows(const typename cx_of<T>::type (&x)[CT],
         if (any_remove) {
             red_s[oc * PP + ky] = m0.x * ar + m0.y * ai;          // Re(conj(m~) y~)
             if (nq_m > 1) { const C2 mm = (oc & 1) ? m2 : m1; red_f[oc * PP + ky] = mm.x * ar + mm.y * ai; }
+            if (MR) {          // MINRES: the same modal sums of the product's INPUT v~ (mac_slab), from the registers
+                T *red_v = red_s + (nq_m > 1 ? 2 : 1) * CT * PP;
+                const T ip2 = (T)1 / ((T)PP * (T)PP);
+                red_v[oc * PP + ky] = ip2 * (m0.x * x[oc].x + m0.y * x[oc].y);
+                if (nq_m > 1) { const C2 mm = (oc & 1) ? m2 : m1; red_v[(CT + oc) * PP + ky] = ip2 * (mm.x * x[oc].x + mm.y * x[oc].y); }
+            }
         }
     }
 }
-template <typename T, typename S, int CT, int PP, int G>
+template <typename T, typename S, int CT, int PP, int G, bool MR = false>
 __device__ __forceinline__ void mac_dispatch(int grp, const typename cx_of<T>::type (&x)[CT], const typename cx_of<S>::type *sp,
                                              const T *s2c, typename cx_of<T>::type *Y, int LD, int ky, typename cx_of<T>::type m0,
                                              typename cx_of<T>::type m1, typename cx_of<T>::type m2, T *red_s, T *red_f,
                                              int any_remove, int nq_m, T &pap) {
     constexpr int WPG = (PP + 31) / 32, GOC = (kPWarps / WPG) < CT ? (kPWarps / WPG) : CT;
-    if (grp == G) mac_rows<T, S, CT, PP, G * CT / GOC, (G + 1) * CT / GOC>(x, sp, s2c, Y, LD, ky, m0, m1, m2, red_s, red_f, any_remove, nq_m, pap);
-    else if constexpr (G + 1 < GOC) mac_dispatch<T, S, CT, PP, G + 1>(grp, x, sp, s2c, Y, LD, ky, m0, m1, m2, red_s, red_f, any_remove, nq_m, pap);
+    if (grp == G) mac_rows<T, S, CT, PP, G * CT / GOC, (G + 1) * CT / GOC, MR>(x, sp, s2c, Y, LD, ky, m0, m1, m2, red_s, red_f, any_remove, nq_m, pap);
+    else if constexpr (G + 1 < GOC) mac_dispatch<T, S, CT, PP, G + 1, MR>(grp, x, sp, s2c, Y, LD, ky, m0, m1, m2, red_s, red_f, any_remove, nq_m, pap);
 }
 
 // ---- per-frequency block product of one k_x slab (Eq.22, Eq.30) + Sigma_eta (L260) + Parseval partials.
@@ -271,7 +277,7 @@ __device__ __forceinline__ void mac_slab(const typename cx_of<T>::type *X, typen
     }
     T pap = (T)0;
     if constexpr (CT > 0) {
-        mac_dispatch<T, S, CT, PP, 0>(grp, x, sp, s2c, Y, LD, ky, m0, m1, m2, red_s, red_f, any_remove, nq_m, pap);
+        mac_dispatch<T, S, CT, PP, 0, MR>(grp, x, sp, s2c, Y, LD, ky, m0, m1, m2, red_s, red_f, any_remove, nq_m, pap);
     } else {
 #pragma unroll 1
         for (int oc = oc_lo; oc < oc_hi; ++oc) {
@@ -296,7 +302,7 @@ __device__ __forceinline__ void mac_slab(const typename cx_of<T>::type *X, typen
         }
     }
     red[grp * P + ky] = pap;
-    if (MR && any_remove) {        // MINRES: the same modal sums of the product's INPUT v~ (every v_k is re-projected, reading G27)
+    if (MR && any_remove && CT == 0) {        // MINRES: the same modal sums of the product's INPUT v~ (every v_k is re-projected, reading G27; CT > 0: in mac_rows)
         T *red_v = red_s + (nq_m > 1 ? 2 : 1) * C * P;
         const T ip2 = (T)1 / ((T)P * (T)P);           // v~ is an unnormalised transform (y~ carries the 1/P^2 folded into the kernel spectra)
         for (int oc = oc_lo; oc < oc_hi; ++oc) {
@@ -310,7 +316,13 @@ __device__ __forceinline__ void mac_slab(const typename cx_of<T>::type *X, typen
 // fixed-order sum of `cnt` values of the slab partial array by one warp
 template <typename T> __device__ __forceinline__ double warp_sum_red(const T *src, int cnt, int lane) {
     T s = (T)0;
-    for (int i = lane; i < cnt; i += 32) s += src[i];
+    for (int i0 = 0; i0 < cnt; i0 += 256) {          // eight loads in flight, added in the order i = lane, lane + 32, ...
+        T v[8];
+#pragma unroll
+        for (int m = 0; m < 8; ++m) { const int i = i0 + lane + 32 * m; v[m] = i < cnt ? src[i] : (T)0; }
+#pragma unroll
+        for (int m = 0; m < 8; ++m) s += v[m];
+    }
     return warp_sum((double)s);
 }
 
@@ -344,6 +356,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
     int *s_nrem = reinterpret_cast<int *>(sGs + 9 * N);
     T *s_s2c = reinterpret_cast<T *>(s_nrem + N + (N & 1));
     unsigned *s_vm = reinterpret_cast<unsigned *>(smem_raw + a.off_vm);
+    T *s_coef = reinterpret_cast<T *>(smem_raw + a.off_upart);        // [C][4] mode coefficients of q (and of v_k: MINRES), single frame
     T *svec = reinterpret_cast<T *>(smem_raw + a.off_vec);
     S2 *sspec = reinterpret_cast<S2 *>(smem_raw + a.off_spec);
     PairRef *ptab = reinterpret_cast<PairRef *>(smem_raw + a.off_ptab);
@@ -465,10 +478,16 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
         unit_fft(act, n);
         if (act) {
             C2 *out = a.T1 + (((size_t)q.f * Ph) * C + q.c) * npad + q.y0;
-            for (int kk = gl; kk < Ph; kk += kGS) {
-                const C2 z1 = bufA[kk], z2 = bufA[kk == 0 ? 0 : P - kk];
-                st_pair(out + (size_t)kk * C * npad, mk<T>((T)0.5 * (z1.x + z2.x), (T)0.5 * (z1.y - z2.y)),
-                        q.two ? mk<T>((T)0.5 * (z1.y + z2.y), (T)-0.5 * (z1.x - z2.x)) : mk<T>((T)0, (T)0));
+            constexpr int NLS = (Ph + kGS - 1) / kGS;          // every load before the first store
+            C2 z1[NLS], z2[NLS];
+#pragma unroll
+            for (int m = 0; m < NLS; ++m) { const int kk = gl + m * kGS; if (kk < Ph) { z1[m] = bufA[kk]; z2[m] = bufA[kk == 0 ? 0 : P - kk]; } }
+#pragma unroll
+            for (int m = 0; m < NLS; ++m) {
+                const int kk = gl + m * kGS;
+                if (kk < Ph)
+                    st_pair(out + (size_t)kk * C * npad, mk<T>((T)0.5 * (z1[m].x + z2[m].x), (T)0.5 * (z1[m].y - z2[m].y)),
+                            q.two ? mk<T>((T)0.5 * (z1[m].y + z2[m].y), (T)-0.5 * (z1[m].x - z2[m].x)) : mk<T>((T)0, (T)0));
             }
         }
     };
@@ -720,7 +739,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                 const int slot = NW - 1 - warp;
                 if (slot < nfree) {
                     for (int tq = lo + slot; tq < hi; tq += nfree) {
-                        const int fr = tq / NQ, q1 = tq - fr * NQ;
+                        const int fr = BATCH ? tq / NQ : 0, q1 = tq - fr * NQ;
                         const T *rd = red + fr * red_sz;
                         double s = 0.0;
                         if (q1 == 0) s = warp_sum_red<T>(rd, Goc * P, lane);
@@ -797,11 +816,16 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                     else if (item < F) { f = item; qq = 0; }
                     else { const int r = item - F; f = fu_lo + r / (NQ - 1); qq = 1 + r % (NQ - 1); }
                 };
-                for (int item0 = NW - 1 - warp; item0 < n_sc; item0 += NB * NW) {
+                // single frame: the warps that hold no row unit this round take the items and, behind a barrier of their own, form
+                // alpha_k and the mode coefficients of every channel (s_coef) while the unit warps are still in stage 1
+                const int nuw = (min(NGS, nu) * kGS + 31) >> 5;             // warps with row units
+                const bool split = !BATCH && MINRES && nuw + 2 <= NW;      // (CG: a row unit forms its few coefficients faster itself)
+                const int NWs = split ? NW - nuw : NW;                      // warps that take items (from the top warp down)
+                for (int item0 = NW - 1 - warp; item0 < n_sc && NW - 1 - warp < NWs; item0 += NB * NWs) {
                     double v[NB][NLD];
 #pragma unroll
                     for (int j = 0; j < NB; ++j) {
-                        const int item = item0 + j * NW;
+                        const int item = item0 + j * NWs;
                         int f = 0, qq = 0;
                         if (item < n_sc) sc_item(item, f, qq);
                         const bool on = item < n_sc && (qq == 0 || a.any_remove);
@@ -811,7 +835,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                     }
 #pragma unroll
                     for (int j = 0; j < NB; ++j) {
-                        const int item = item0 + j * NW;
+                        const int item = item0 + j * NWs;
                         if (item < n_sc) {
                             int f, qq;
                             sc_item(item, f, qq);
@@ -824,10 +848,38 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                         }
                     }
                 }
+                if (split) {
+                    if (warp >= nuw) {
+                        asm volatile("bar.sync 1, %0;" ::"r"(NWs * 32) : "memory");
+                        const double *sc = scal;
+                        if (warp == NW - 1 && !pre) {                            // alpha_k (frame 0)
+                            double al;
+                            if (MINRES) al = minres_alpha(sc);
+                            else { const double rho = sc[SC_RHO], pq = sc[SC_PQ]; al = (rho > 0.0 && pq > 0.0) ? div_as<T>(rho, pq) : 0.0; }   // breakdown: freeze (reading G16)
+                            if (lane == 0) { scal[SC_ALPHA] = al; if (b == 0) a.alpha[0] = al; }
+                        }
+                        if (warp == NW - 2) for (int ch = lane; ch < C; ch += 32) {       // mode coefficients of channel ch (Eq.36)
+                            const int w = ch >> 1, comp = ch & 1, nr = s_nrem[w];
+                            const double *S0 = sc + SC_HEAD, *S1 = S0 + C;
+                            const double tq[3] = {S0[2 * w], S0[2 * w + 1], S1[2 * w] + S1[2 * w + 1]};
+                            double d0, d2;
+                            modal_coef(sGs + w * 9, tq, nr, comp, d0, d2);
+                            s_coef[ch * 4 + 0] = (comp < nr) ? (T)d0 : (T)0;
+                            s_coef[ch * 4 + 1] = (2 < nr) ? (T)d2 : (T)0;
+                            if (MINRES) {
+                                const double *V0 = sc + SCM, *V1 = V0 + C;
+                                const double tp[3] = {V0[2 * w], V0[2 * w + 1], V1[2 * w] + V1[2 * w + 1]};
+                                modal_coef(sGs + w * 9, tp, nr, comp, d0, d2);
+                                s_coef[ch * 4 + 2] = (comp < nr) ? (T)d0 : (T)0;
+                                s_coef[ch * 4 + 3] = (2 < nr) ? (T)d2 : (T)0;
+                            }
+                        }
+                    }
+                }
                 __syncthreads();
-                // alpha_k is recorded for the next phase C / the tail; every row unit derives alpha and its own mode
-                // coefficients from the sums itself (a few fp64 operations per lane beat a serial section + a barrier)
-                if (!pre) {
+                // alpha_k is recorded for the next phase C / the tail; (batch, or too few free warps) every row unit derives alpha
+                // and its own mode coefficients from the sums itself
+                if (!pre && !split) {
                     if (MINRES && BATCH) {                                       // (single frame: recorded in stage 2 below)
                         for (int f0 = gs & ~1; f0 < F; f0 += kPThreads / kGS) {   // one 16-lane group per frame; the two groups of a
                             const int f = f0 + (gs & 1);                         // warp go through the full-mask shuffles together
@@ -850,20 +902,28 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
             // stage 2: q' = M_s q, CG vector updates, r.r partial, the new residual rows -> bufA -> forward x-FFT -> T1
             double rr = 0.0;
             double al_mr = 0.0;                      // MINRES: alpha_k of the unit's frame, one WFS term per lane of the group
+            const int nuw2 = (min(NGS, nu) * kGS + 31) >> 5;
+            const bool from_tab = !BATCH && MINRES && nuw2 + 2 <= NW;              // alpha and the coefficients were formed by the free warps
             if (MINRES && !pre) {
-                al_mr = minres_alpha(scal + q.f * SB);                       // (batch: bitwise the value recorded in SC_ALPHA above)
-                if (!BATCH && rnd == 0 && tid == 0) { scal[SC_ALPHA] = al_mr; if (b == 0) a.alpha[0] = al_mr; }
+                if (from_tab) al_mr = scal[SC_ALPHA];
+                else {
+                    al_mr = minres_alpha(scal + q.f * SB);                       // (batch: bitwise the value recorded in SC_ALPHA above)
+                    if (!BATCH && rnd == 0 && tid == 0) { scal[SC_ALPHA] = al_mr; if (b == 0) a.alpha[0] = al_mr; }
+                }
             }
             if (act) {
                 const double *sc = scal + q.f * SB;
                 const double rho_k = sc[SC_RHO], pq_k = sc[SC_PQ];
-                const double al = (!pre && rho_k > 0.0 && pq_k > 0.0) ? div_as<T>(rho_k, pq_k) : 0.0;   // = sc[SC_ALPHA]
+                double al;
+                if (from_tab) al = pre ? 0.0 : sc[SC_ALPHA];
+                else al = (!pre && rho_k > 0.0 && pq_k > 0.0) ? div_as<T>(rho_k, pq_k) : 0.0;   // = sc[SC_ALPHA]
                 const T alpha = (T)al, beta = (T)sc[SC_BETA];
                 const bool apply = a.mode == PM_APPLY;
                 const bool upd = sc[SC_UPD] != 0.0, step = al != 0.0 && !apply;
                 // mode coefficients (Z^T Z)^-1 Z^T q of this unit's WFS from the channel sums (Eq.36)
                 T c0 = (T)0, c2 = (T)0;
-                {
+                if (from_tab) { c0 = s_coef[q.c * 4]; c2 = s_coef[q.c * 4 + 1]; }
+                else {
                     const double *S0 = sc + SC_HEAD, *S1 = sc + SC_HEAD + C;
                     const double tq[3] = {S0[2 * q.w], S0[2 * q.w + 1], S1[2 * q.w] + S1[2 * q.w + 1]};
                     const int nr = s_nrem[q.w];
@@ -874,10 +934,42 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                 }
                 const unsigned vm = s_vm[i * kGS + gl];
                 const T *ub = dense(i, q, 3);
+
                 // x, r, p of the unit: shared memory (vec_smem) or the dense global rows; separate code so that the
                 // loads and stores are LDS/STS resp. LDG/STG, not generic
-                auto update_rows = [&](T *ux, T *ur, T *up) {
+                auto update_rows = [&](T *ux, T *ur, T *up, const bool steady) {
                     constexpr int NX = (P / 2 + kGS) / kGS;              // columns per lane, n <= P/2 + 1
+                    if (steady) {
+                        // the steady-state iteration (k >= 1, no breakdown) on shared-memory rows, branch-free: every column x < n
+                        // is processed; outside the pupil the rows hold zeros and stay zero (q is masked there: W_s), so the
+                        // arithmetic of a valid element is that of the general code below, operation by operation
+#pragma unroll
+                        for (int m = 0; m < NX; ++m) {
+                            const int xp = gl + m * kGS;
+                            if (xp < n) {
+                                const C2 z = bufA[xp];
+                                T nr[2];
+#pragma unroll
+                                for (int row = 0; row < 2; ++row) {
+                                    const bool valid = (vm >> (row * 16 + m)) & 1u;
+                                    const T coord = ((q.comp ? (T)(q.y0 + row) : (T)xp) - half_n) * dd;
+                                    const T qm = (row ? -z.y : z.x) - (c0 + c2 * coord);
+                                    const T qp = valid ? qm : (T)0;
+                                    const int idx = row * n + xp;
+                                    T rv = ur[idx];
+                                    const T pv = rv + beta * up[idx];
+                                    up[idx] = pv;
+                                    ux[idx] = ux[idx] + alpha * pv;
+                                    rv -= alpha * qp;
+                                    ur[idx] = rv;
+                                    rr += (double)rv * (double)rv;
+                                    nr[row] = rv;
+                                }
+                                bufA[xp] = mk<T>(nr[0], nr[1]);
+                            }
+                        }
+                        return;
+                    }
                     constexpr int NH = BATCH ? (NX + 1) / 2 : 1;         // two halves: every load of a half is issued before its
                                                                          // first store (a store between two loads serialises them:
                                                                          // one L2 round trip per element with the rows in global memory)
@@ -937,13 +1029,15 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                 };
                 // MINRES (one Lanczos step + the x / w update of the PREVIOUS iteration, whose rotation needed |u|): rows x, v_{k-1},
                 // u_{k-1} (v_k = u_{k-1} / beta_k, re-projected: reading G27), w_{k-1}, w_{k-2}
-                auto update_rows_mr = [&](T *ux, T *uvo, T *uvc, T *uw1, T *uw2) {
+                auto update_rows_mr = [&](T *ux, T *uvo, T *uvc, T *uw1, T *uw2, const bool steady_ok) {
                     const double *st = sc + MRS;
                     const bool frozen = st[MR_FROZEN] != 0.0, first = k == 0, pon = st[MR_PON] != 0.0;
+                    const bool steady = steady_ok && !frozen && !first && pon;
                     const T alm = (T)al_mr, betak = (T)st[MR_BETA], ib = (T)st[MR_INVBETA];
                     const T peps = (T)st[MR_PEPS], pdelta = (T)st[MR_PDELTA], pinvg = (T)st[MR_PINVG], pphi = (T)st[MR_PPHI];
                     T cv0 = (T)0, cv2 = (T)0;                             // mode coefficients of v_k
-                    {
+                    if (from_tab) { cv0 = s_coef[q.c * 4 + 2]; cv2 = s_coef[q.c * 4 + 3]; }
+                    else {
                         const double *V0 = sc + SCM, *V1 = V0 + C;
                         const double tp[3] = {V0[2 * q.w], V0[2 * q.w + 1], V1[2 * q.w] + V1[2 * q.w + 1]};
                         const int nr = s_nrem[q.w];
@@ -953,6 +1047,39 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                         cv2 = (2 < nr) ? (T)d2 : (T)0;
                     }
                     constexpr int NX = (P / 2 + kGS) / kGS;              // columns per lane
+                    if (steady) {
+                        // the steady-state iteration (k >= 1, a pending x / w update, no breakdown) on shared-memory rows, branch-free as
+                        // in update_rows: outside the pupil the five rows hold zeros and stay zero (q and the projection of v_k are
+                        // masked there); a valid element goes through the operations of the general code below
+#pragma unroll
+                        for (int m = 0; m < NX; ++m) {
+                            const int xp = gl + m * kGS;
+                            if (xp < n) {
+                                const C2 z = bufA[xp];
+                                T nr[2];
+#pragma unroll
+                                for (int row = 0; row < 2; ++row) {
+                                    const bool valid = (vm >> (row * 16 + m)) & 1u;
+                                    const int idx = row * n + xp;
+                                    const T coord = ((q.comp ? (T)(q.y0 + row) : (T)xp) - half_n) * dd;
+                                    const T vo = uvo[idx];
+                                    const T w1v = uw1[idx];
+                                    const T w = (vo - peps * uw2[idx] - pdelta * w1v) * pinvg;
+                                    ux[idx] = ux[idx] + pphi * w;
+                                    uw2[idx] = w1v; uw1[idx] = w;
+                                    const T vpm = uvc[idx] * ib - (cv0 + cv2 * coord);
+                                    const T qm = (row ? -z.y : z.x) - (c0 + c2 * coord);
+                                    const T vp = valid ? vpm : (T)0, qp = valid ? qm : (T)0;
+                                    const T uv = qp - alm * vp - betak * vo;
+                                    uvo[idx] = vp; uvc[idx] = uv;
+                                    rr += (double)uv * (double)uv;
+                                    nr[row] = uv;
+                                }
+                                bufA[xp] = mk<T>(nr[0], nr[1]);
+                            }
+                        }
+                        return;
+                    }
                     constexpr int NH = (NX + 1) / 2;                     // two halves (five vectors: all columns at once spill);
                                                                          // every load of a half is issued before its first store
 #pragma unroll
@@ -1007,17 +1134,17 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(PArgs<T, S> a) {
                 if (MINRES && !pre) {
                     if (a.vec_smem) {
                         T *base = svec + (size_t)i * NVEC * 2 * n;
-                        update_rows_mr(base, base + 2 * n, base + 4 * n, base + 6 * n, base + 8 * n);
+                        update_rows_mr(base, base + 2 * n, base + 4 * n, base + 6 * n, base + 8 * n, true);
                     } else {
                         const size_t o = (((size_t)q.f * C + q.c) * npad + q.y0) * n;
-                        update_rows_mr(a.xd + o, a.rd + o, a.pd + o, a.w1d + o, a.w2d + o);
+                        update_rows_mr(a.xd + o, a.rd + o, a.pd + o, a.w1d + o, a.w2d + o, false);
                     }
                 } else if (a.vec_smem) {
                     T *base = svec + (size_t)i * NVEC * 2 * n;
-                    update_rows(base, base + 2 * n, base + 4 * n);
+                    update_rows(base, base + 2 * n, base + 4 * n, !pre && !apply && upd && step);
                 } else {
                     const size_t o = (((size_t)q.f * C + q.c) * npad + q.y0) * n;
-                    update_rows(a.xd + o, a.rd + o, a.pd + o);
+                    update_rows(a.xd + o, a.rd + o, a.pd + o, false);
                 }
             }
             rr = group_sum(rr);

@@ -147,7 +147,7 @@ static int persist_prepare(tomo_plan *pl) {
     ps->off_tab = (int)(off = align16(off));
     off += (size_t)m.n_wfs * (9 * sizeof(double) + sizeof(int)) + 8 + (size_t)(m.C + 2) * E + 16;
     ps->off_upart = (int)(off = align16(off));
-    off += (size_t)maxu * sizeof(double);
+    off += std::max((size_t)maxu * sizeof(double), (size_t)m.C * 4 * E);      // [C][4] mode coefficients (single-frame instance)
     ps->off_vm = (int)(off = align16(off));
     off += (size_t)maxu * kGS * sizeof(unsigned);
     ps->off_ptab = (int)(off = align16(off));
