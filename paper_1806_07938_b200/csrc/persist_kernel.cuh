@@ -207,30 +207,37 @@ __device__ __forceinline__ void mac_rows(const typename cx_of<T>::type (&x)[CT],
                                          int any_remove, int nq_m, T &pap) {
     typedef typename cx_of<T>::type C2;
     typedef typename cx_of<S>::type S2;
+    // input channel outermost: the HI - LO outputs of the group advance together (2 (HI - LO) independent accumulator chains);
+    // the terms of an output still arrive in the order c_in = 0 .. C-1
+    T ar[HI - LO], ai[HI - LO];
 #pragma unroll
-    for (int oc = LO; oc < HI; ++oc) {
-        const T s2 = s2c[oc];
-        T ar = s2 * x[oc].x, ai = s2 * x[oc].y;
+    for (int o = 0; o < HI - LO; ++o) { const T s2 = s2c[LO + o]; ar[o] = s2 * x[LO + o].x; ai[o] = s2 * x[LO + o].y; }
 #pragma unroll
-        for (int ci = 0; ci < CT; ++ci) {
+    for (int ci = 0; ci < CT; ++ci) {
+#pragma unroll
+        for (int o = 0; o < HI - LO; ++o) {
+            const int oc = LO + o;
             const int lo = ci < oc ? ci : oc, hi = ci < oc ? oc : ci;
             const S2 s = sp[(lo * CT - (lo * (lo - 1)) / 2 + hi - lo) * PP];
             const T sr = (T)s.x, si = (T)s.y;
-            // four dependent-free FMAs per complex product ("ar += a*b - c*d" compiles to FMUL + FFMA + FADD)
             if (ci < oc) {           // conjugate of the stored block
-                ar = fma(sr, x[ci].x, ar); ar = fma(si, x[ci].y, ar);
-                ai = fma(sr, x[ci].y, ai); ai = fma(-si, x[ci].x, ai);
+                ar[o] = fma(sr, x[ci].x, ar[o]); ar[o] = fma(si, x[ci].y, ar[o]);
+                ai[o] = fma(sr, x[ci].y, ai[o]); ai[o] = fma(-si, x[ci].x, ai[o]);
             } else {
-                ar = fma(sr, x[ci].x, ar); ar = fma(-si, x[ci].y, ar);
-                ai = fma(sr, x[ci].y, ai); ai = fma(si, x[ci].x, ai);
+                ar[o] = fma(sr, x[ci].x, ar[o]); ar[o] = fma(-si, x[ci].y, ar[o]);
+                ai[o] = fma(sr, x[ci].y, ai[o]); ai[o] = fma(si, x[ci].x, ai[o]);
             }
         }
-        Y[oc * LD + ky] = mk<T>(ar, -ai);
-        pap += x[oc].x * ar + x[oc].y * ai;                       // Re(conj(p~) y~)
+    }
+#pragma unroll
+    for (int o = 0; o < HI - LO; ++o) {
+        const int oc = LO + o;
+        Y[oc * LD + ky] = mk<T>(ar[o], -ai[o]);
+        pap += x[oc].x * ar[o] + x[oc].y * ai[o];                       // Re(conj(p~) y~)
         if (any_remove) {
-            red_s[oc * PP + ky] = m0.x * ar + m0.y * ai;          // Re(conj(m~) y~)
-            if (nq_m > 1) { const C2 mm = (oc & 1) ? m2 : m1; red_f[oc * PP + ky] = mm.x * ar + mm.y * ai; }
-            if (MR) {          // MINRES: the same modal sums of the product's INPUT v~ (mac_slab), from the registers
+            red_s[oc * PP + ky] = m0.x * ar[o] + m0.y * ai[o];          // Re(conj(m~) y~)
+            if (nq_m > 1) { const C2 mm = (oc & 1) ? m2 : m1; red_f[oc * PP + ky] = mm.x * ar[o] + mm.y * ai[o]; }
+            if (MR) {
                 T *red_v = red_s + (nq_m > 1 ? 2 : 1) * CT * PP;
                 const T ip2 = (T)1 / ((T)PP * (T)PP);
                 red_v[oc * PP + ky] = ip2 * (m0.x * x[oc].x + m0.y * x[oc].y);
