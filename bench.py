@@ -259,6 +259,10 @@ def main():
     t0 = time.perf_counter()
     plan = tomo.TomoPlan(cfg, max_batch=B, precision=prec, solver=solver)
     t_plan = time.perf_counter() - t0
+    # the solver that RUNS the plan (decided by the library at upload: a plan the persistent kernel cannot take falls back to the
+    # multi-kernel solver, e.g. n = 128 with max_batch 16 does not fit its shared-memory layout); every number below is labelled with it
+    sv, solver_note = plan.solver_in_use()
+    solver_used = "persistent" if sv == tomo.TOMO_SOLVER_PERSISTENT else "multikernel"
     sigma2 = float(plan.noise()[0][0])
     # every rank (replica) gets its own frames: seed offset by rank
     data = screens.generate(cfg, sigma2, n_frames=B, seed_offset=10 * rank)
@@ -330,7 +334,7 @@ def main():
     clocks = sampler.stop()
 
     # per-kernel device times of the multi-kernel loop (CUDA events after every kernel, on the launch stream)
-    kt = plan.time_kernels(B, n_iter, stream=stream) if args.solver == "multikernel" else None
+    kt = plan.time_kernels(B, n_iter, stream=stream) if solver_used == "multikernel" else None
     n, C, P = cfg.n, 2 * cfg.n_wfs, plan.P
     Ph, Ns, npair = P // 2 + 1, 2 * cfg.n_wfs * plan.n_vs, C * (C + 1) // 2
     E = 4 if prec == tomo.TOMO_F32 else 8
@@ -352,7 +356,7 @@ def main():
                 "state": "in situ inside the iteration loop (spectra L2-resident after the first iteration)"}
     f_iter = 2 * C * (n * 2.5 * P * np.log2(P) + Ph * 5 * P * np.log2(P)) + 8 * C * C * P * Ph      # SURVEY 8(d), per frame
     fp32_peak = 148 * 128 * 2 * 1.965e9                                                             # nominal FMA peak, DESIGN.md 6
-    if args.solver == "persistent":
+    if solver_used == "persistent":
         # the dominant kernel is the persistent solver itself: device time of the launch alone (CUDA events on the stream)
         reps = max(3, min(args.steps, 50))
         k_ms = plan.time_solver(d_slopes, B, n_iter, reps, stream=stream, minres=minres)
@@ -375,7 +379,7 @@ def main():
     dev_meas = tomo.measure_device(0, 5, stream=stream)
     npairs_rows = (n + 1) // 2
     exch = Ph * C * 2 * npairs_rows * 2 * E                       # one row <-> column exchange buffer of one frame
-    if args.solver == "persistent":
+    if solver_used == "persistent":
         # per frame-iteration through L2: T1 written + read, T1p read + written, T2 written + read (spectra sit in shared memory)
         l2_bytes_iter = B * 6 * exch
         l2_what = "T1, T1p, T2 exchange buffers: 6 passes per frame-iteration (spectra pinned in shared memory)"
@@ -395,7 +399,7 @@ def main():
     line = {"metric": METRIC, "value": value, "unit": "reconstructions/s", "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": args.precision, "data": "synthetic",
-            "config": workload_config(cfg, plan.P, plan.P_os, n_iter, B, args.solver, args.method, world),
+            "config": workload_config(cfg, plan.P, plan.P_os, n_iter, B, solver_used, args.method, world),
             "us_per_cg_iteration": us_iter, "ms_per_step_n_iter0": ms_step0, "ms_per_step_l2_warm": ms_step_warm,
             "reconstructions_per_s_l2_warm": world * B * 1e3 / ms_step_warm,
             "iteration_roofline": iter_roof, "l2_roofline": l2_roof, "roofline": roof,
@@ -403,6 +407,8 @@ def main():
                     "h2d_bytes_per_step": int(h_slopes.numel() * 4), "d2h_bytes_per_step": int(out_h.numel() * 4)},
             "gpu_launches": launches * args.steps, "launches_per_step": launches, "clocks": clocks,
             "plan_build_s": t_plan, "device_bytes": plan.stats()["device_bytes"]}
+    if solver_used != args.solver:
+        line["solver_fallback"] = {"requested": args.solver, "used": solver_used, "reason": solver_note}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         step, desc, cores, extrapolated = oracle_setup(cfg, n_iter, whole=False)
         sec = statistics.median(step() for _ in range(3))

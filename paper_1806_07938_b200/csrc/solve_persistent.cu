@@ -132,38 +132,44 @@ static int persist_prepare(tomo_plan *pl) {
     // row-unit slots per round: as few rounds as 32 groups allow, then as few slots as those rounds need
     const int rounds = std::max(1, (maxu + kPThreads / kGS - 1) / (kPThreads / kGS));
     ps->ngs = std::min(kPThreads / kGS, (((maxu + rounds - 1) / rounds) + 1) & ~1);
-    ps->fb = (F > 1 && 2 * m.C * fb <= kPThreads) ? 2 : 1;      // frames per slab pass of the batch instance
-    size_t off = (size_t)m.P * 2 * E;
-    ps->off_ms = (int)(off = align16(off));
-    off += (size_t)ps->nq_m * m.P * 2 * E;
-    ps->off_ms2 = (int)(off = align16(off));
-    off += (size_t)ps->nq_m * m.P * 2 * E + 32;      // + the CTA's row of the slab segment table
-    ps->off_work = (int)(off = align16(off));
-    off += std::max((size_t)2 * ps->fb * m.C * LD, (size_t)ps->ngs * (m.P + LD)) * 2 * E;
-    ps->off_red = (int)(off = align16(off));
-    off += (size_t)ps->fb * (Goc + 4 * m.C) * m.P * E;
-    ps->off_scal = (int)(off = align16(off));
-    off += (size_t)F * ps->SB * sizeof(double);
-    ps->off_tab = (int)(off = align16(off));
-    off += (size_t)m.n_wfs * (9 * sizeof(double) + sizeof(int)) + 8 + (size_t)(m.C + 2) * E + 16;
-    ps->off_upart = (int)(off = align16(off));
-    off += std::max((size_t)maxu * sizeof(double), (size_t)m.C * 4 * E);      // [C][4] mode coefficients (single-frame instance)
-    ps->off_vm = (int)(off = align16(off));
-    off += (size_t)maxu * kGS * sizeof(unsigned);
-    ps->off_ptab = (int)(off = align16(off));
-    off += (size_t)m.C * m.C * sizeof(PairRef);
-    ps->off_unit = (int)(off = align16(off));
-    off += (size_t)std::max(maxu, 1) * sizeof(UnitRec);
-    off = align16(off);
-    const size_t spec_bytes = (size_t)m.n_pair * m.P * 2 * SE, vec_bytes = (size_t)maxu * 6 * m.n * E, vec_bytes_mr = (size_t)maxu * 10 * m.n * E;
-    // the spectra slice has priority for the shared memory that is left, then the CG vectors of the CTA's row units
-    ps->off_spec = (int)off;
-    ps->spec_smem = off + spec_bytes <= (size_t)max_smem;
-    if (ps->spec_smem) off = align16(off + spec_bytes);
-    ps->off_vec = (int)off;
-    ps->vec_smem = off + vec_bytes <= (size_t)max_smem;
-    ps->vec_smem_mr = ps->vec_smem && (off + vec_bytes_mr <= (size_t)max_smem);      // MINRES keeps five row vectors per unit
-    if (ps->vec_smem) off = align16(off + (ps->vec_smem_mr ? vec_bytes_mr : vec_bytes));
+    // frames per slab pass of the batch instance: two when the FFT passes have the threads for it AND the doubled pass buffers
+    // fit (P = 256 with 16 frames: they do not, and one frame per pass keeps the plan on the persistent kernel)
+    size_t off = 0;
+    for (int fbp = (F > 1 && 2 * m.C * fb <= kPThreads) ? 2 : 1; fbp >= 1; --fbp) {
+        ps->fb = fbp;
+        off = (size_t)m.P * 2 * E;
+        ps->off_ms = (int)(off = align16(off));
+        off += (size_t)ps->nq_m * m.P * 2 * E;
+        ps->off_ms2 = (int)(off = align16(off));
+        off += (size_t)ps->nq_m * m.P * 2 * E + 32;      // + the CTA's row of the slab segment table
+        ps->off_work = (int)(off = align16(off));
+        off += std::max((size_t)2 * ps->fb * m.C * LD, (size_t)ps->ngs * (m.P + LD)) * 2 * E;
+        ps->off_red = (int)(off = align16(off));
+        off += (size_t)ps->fb * (Goc + 4 * m.C) * m.P * E;
+        ps->off_scal = (int)(off = align16(off));
+        off += (size_t)F * ps->SB * sizeof(double);
+        ps->off_tab = (int)(off = align16(off));
+        off += (size_t)m.n_wfs * (9 * sizeof(double) + sizeof(int)) + 8 + (size_t)(m.C + 2) * E + 16;
+        ps->off_upart = (int)(off = align16(off));
+        off += std::max((size_t)maxu * sizeof(double), (size_t)m.C * 4 * E);      // [C][4] mode coefficients (single-frame instance)
+        ps->off_vm = (int)(off = align16(off));
+        off += (size_t)maxu * kGS * sizeof(unsigned);
+        ps->off_ptab = (int)(off = align16(off));
+        off += (size_t)m.C * m.C * sizeof(PairRef);
+        ps->off_unit = (int)(off = align16(off));
+        off += (size_t)std::max(maxu, 1) * sizeof(UnitRec);
+        off = align16(off);
+        const size_t spec_bytes = (size_t)m.n_pair * m.P * 2 * SE, vec_bytes = (size_t)maxu * 6 * m.n * E, vec_bytes_mr = (size_t)maxu * 10 * m.n * E;
+        // the spectra slice has priority for the shared memory that is left, then the CG vectors of the CTA's row units
+        ps->off_spec = (int)off;
+        ps->spec_smem = off + spec_bytes <= (size_t)max_smem;
+        if (ps->spec_smem) off = align16(off + spec_bytes);
+        ps->off_vec = (int)off;
+        ps->vec_smem = off + vec_bytes <= (size_t)max_smem;
+        ps->vec_smem_mr = ps->vec_smem && (off + vec_bytes_mr <= (size_t)max_smem);      // MINRES keeps five row vectors per unit
+        if (ps->vec_smem) off = align16(off + (ps->vec_smem_mr ? vec_bytes_mr : vec_bytes));
+        if (off <= (size_t)max_smem) break;
+    }
     if (off > (size_t)max_smem) { delete ps; set_error("persistent solver: problem too large for shared memory"); return TOMO_EUNSUPPORTED; }
     ps->smem = off;
 

@@ -236,7 +236,8 @@ def test_cfg4_persistent_product_steps_and_moao_projection_against_the_matrix_fr
 
 
 # ------------------------------------------------------------------------------------------------ batch instance
-@pytest.mark.parametrize("name,frames", [("cfg3", (3, 5)), ("cfg4", (3,)), ("cfg5_n128", (2,))], ids=["cfg3-P160-C12", "cfg4-P160-C16", "n128-P256"])
+@pytest.mark.parametrize("name,frames", [("cfg3", (3, 5)), ("cfg4", (3,)), ("cfg5_n128", (2,)), ("cfg5_n128", (16,))],
+                         ids=["cfg3-P160-C12", "cfg4-P160-C16", "n128-P256", "n128-P256-b16-one-frame-per-pass"])
 def test_batch_instance_equals_single_solves_bitwise(name, frames):
     """Batch path at full size: with several frames the slab passes are balanced over the CTAs and some spectra are read
     through L2 instead of shared memory.  Same arithmetic in the same order, so every frame must equal its single-frame
